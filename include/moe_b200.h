@@ -1,0 +1,174 @@
+/* moe_b200.h -- C ABI of the B200-native (sm_100a) routed-expert MoE layer, forward and backward.
+ *
+ * What is computed: the hot path of PithTrain's MoE training step on one GPU
+ * (BASELINE.json:north_star; §3.2 "MoE fwd/bwd have data-dependent
+ * per-expert shapes", "fused SwiGLU fwd/bwd", "FP8 quantization"; App. B.2 "the
+ * top-k expert IDs and their gating weights", "non-negative and sum to 1 over the top-k").  The paper
+ * prints no equation for the layer; the exact arithmetic is the reading R1..R9 of SURVEY.md §8(c),
+ * restated in DESIGN.md, and each entry point below names the R-step it implements.
+ *
+ * Conventions (all entry points)
+ *  - Every pointer is a DEVICE pointer owned by the caller unless its name ends in `_host`.
+ *    The library allocates no device memory and keeps no global state besides lazily resolved
+ *    driver entry points.  Scratch comes from the caller (`ws`), sized by moe_workspace_bytes.
+ *  - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream);
+ *    calls return without synchronising.  Per-expert counts never visit the host.
+ *  - Row-major, innermost dimension contiguous, base pointers 16-byte aligned.
+ *  - Return value: MOE_OK or a negative moe_status; on error nothing has been enqueued.
+ *    No exceptions, no aborts, no printing.  Inputs must be finite.
+ *  - Activation / weight element type follows cfg->dtype: 0 = fp32, 1 = bf16, 2 = bf16 I/O with
+ *    e4m3 block-scaled expert GEMMs.  Logits, gating weights and their gradients are always fp32.
+ *  - Permuted-row tensors have TK_pad = moe_padded_rows(cfg) rows: expert group e occupies rows
+ *    [offsets[e], offsets[e] + counts[e]) and starts at a multiple of cfg->row_align; padding rows
+ *    map to -1 in perm_to_flat and hold zeros.  The tensor-core (bf16 / fp8) GEMMs require
+ *    row_align to be a multiple of 128; the fp32 path accepts any row_align >= 1.
+ */
+#ifndef MOE_B200_H
+#define MOE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct moe_config_t {
+  int32_t T, H, E, K, F;       /* tokens, hidden, routed experts, top-k, expert FFN width             */
+  int32_t n_group, topk_group; /* 1,1 = no group limiting (R3); E % n_group == 0; n_group <= 32        */
+  int32_t score_fn;            /* 0 = softmax, 1 = sigmoid (R2)                                        */
+  int32_t group_score;         /* 0 = max, 1 = sum of the two largest keys in the group (R3)           */
+  int32_t renorm;              /* 1 = divide the selected weights by their sum (R5)                    */
+  float routed_scale;          /* multiplies w after renormalisation (R5)                              */
+  int32_t has_bias;            /* selection-only per-expert bias b[E], no gradient (R2)                */
+  int32_t F_shared;            /* 0 = no shared expert (R7)                                            */
+  int32_t dtype;               /* 0 = fp32, 1 = bf16, 2 = fp8-e4m3 block-scaled GEMMs with bf16 I/O    */
+  int32_t fp8_scale_mode;      /* 0 = fp32 amax/448, 1 = power of two (R9)                             */
+  int32_t row_align;           /* expert groups start at multiples of this many rows (>= 1)            */
+} moe_config_t;
+
+enum moe_status {
+  MOE_OK = 0,
+  MOE_ERR_INVALID_ARG = -1, /* NULL where a pointer is required, non-positive size, bad enum    */
+  MOE_ERR_UNSUPPORTED = -2, /* valid in principle, not implemented for this shape / dtype        */
+  MOE_ERR_WORKSPACE = -3,   /* reserved                                                          */
+  MOE_ERR_CUDA = -4         /* a CUDA runtime / driver call failed (launch error, no sm_100 GPU) */
+};
+
+/* Text for a status code (static storage). */
+const char* moe_status_string(int32_t status);
+
+/* Library version as major*10000 + minor*100 + patch. */
+int32_t moe_version(void);
+
+/* Upper bound on permuted rows: T*K if row_align == 1, else (T*K + E*(row_align-1)) rounded up to
+ * row_align.  Returns < 0 on an invalid config. */
+int64_t moe_padded_rows(const moe_config_t* cfg);
+
+/* Bytes of scratch (`ws`, contents undefined between calls) and of saved-for-backward context
+ * (`ctx`, written by moe_layer_fwd, read by moe_layer_bwd) for this config.  Both 256-byte multiples. */
+int32_t moe_workspace_bytes(const moe_config_t* cfg, size_t* ws_bytes, size_t* ctx_bytes);
+
+/* R2..R5.  Top-k routing from fp32 logits.
+ *   logits [T,E] fp32; bias [E] fp32 or NULL (required iff cfg->has_bias)
+ *   topk_idx [T,K] int32: slot j holds the j-th largest selection key, ties -> lower expert index
+ *   topk_w   [T,K] fp32 gating weights (bias never enters w)
+ * Selection key: softmax -> z (+ b); sigmoid -> fp32(1/(1+exp(-z)) evaluated in fp64) + b in fp32.
+ * Group limiting: keep topk_group of n_group contiguous groups by group score; others -> -inf.
+ * UNSUPPORTED: E > 1024, K > 32, n_group > 32, K > topk_group * E / n_group. */
+int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
+                  float* topk_w, void* stream);
+
+/* R6.  Histogram, exclusive scan, stable counting sort of flat positions
+ * p = t*K + j by expert (no atomics; deterministic), then the row gather Xp[r] = X[perm_to_flat[r] / K].
+ *   X [T,H] (cfg->dtype element type) or NULL to build the maps only (then Xp is ignored)
+ *   topk_idx [T,K]; counts [E]; offsets [E+1]; perm_to_flat [TK_pad] (-1 on padding rows and on rows
+ *   >= offsets[E]); flat_to_perm [T*K]; Xp [TK_pad,H] (padding rows zero; rows >= offsets[E] untouched)
+ *   ws: scratch of at least moe_workspace_bytes().  */
+int32_t moe_permute(const moe_config_t* cfg, const void* X, const int32_t* topk_idx, int32_t* counts,
+                    int32_t* offsets, int32_t* perm_to_flat, int32_t* flat_to_perm, void* Xp, void* ws,
+                    void* stream);
+
+/* R7, one grouped GEMM: for every expert e and row r in [offsets[e], offsets[e+1]):
+ *   C[r, n] = sum_k A[r, k] * B[e][n, k]         A [TK_pad,Kdim], B [E,N,Kdim], C [TK_pad,N]
+ * fp32 accumulation; C in the element type of A.  dtype 2: A and B are e4m3 codes (uint8) with
+ * a_scales [TK_pad, Kdim/128] fp32 and b_scales [E, ceil(N/128), Kdim/128] fp32, C is bf16.
+ * Rows >= offsets[E] are not touched.  Requirements for dtype 1, 2: row_align % 128 == 0, Kdim % 64 == 0
+ * (dtype 2: Kdim % 128 == 0), N % 8 == 0.  */
+int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int32_t Kdim, const void* A, const void* B,
+                             const int32_t* offsets, void* C, const void* a_scales, const void* b_scales,
+                             void* ws, void* stream);
+
+/* R8, the two gradients of C = A * B[e]^T (either output may be NULL = skipped; this is the split
+ * that a delayed weight-gradient schedule needs):
+ *   dA[r, k]    = sum_n dC[r, n] * B[e][n, k]                       (dgrad)   dA [TK_pad,Kdim]
+ *   dB[e][n, k] = sum_{r in e} dC[r, n] * A[r, k]                   (wgrad)   dB [E,N,Kdim], overwritten;
+ *                                                                   an empty expert gets exact zeros
+ * Padding rows of dC and A must be zero (they are when produced by this library).  bf16 / fp32 only. */
+int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int32_t Kdim, const void* dC, const void* A,
+                             const void* B, const int32_t* offsets, void* dA, void* dB, void* ws,
+                             void* stream);
+
+/* R7 SwiGLU ([34]):  a[r,f] = silu(gu[r,f]) * gu[r,F+f],  gu [rows,2F] = [gate | up]. */
+int32_t moe_swiglu(const moe_config_t* cfg, const void* gu, void* a, int64_t rows, void* stream);
+
+/* R8 SwiGLU backward: dgu[r,f] = da*u*s*(1+g*(1-s)), dgu[r,F+f] = da*g*s with s = sigmoid(g). */
+int32_t moe_swiglu_bwd(const moe_config_t* cfg, const void* gu, const void* da, void* dgu, int64_t rows,
+                       void* stream);
+
+/* R7 combine:  Y[t,:] = sum_{j=0..K-1} topk_w[t,j] * y[flat_to_perm[t*K+j],:]  (+ shared_out[t,:]),
+ * fp32 accumulation in ascending j, one rounding to the output type. */
+int32_t moe_unpermute_combine(const moe_config_t* cfg, const void* y, const float* topk_w,
+                              const int32_t* flat_to_perm, const void* shared_out, void* Y, void* stream);
+
+/* R9 quantisers ([22]).  Input is the bf16 tensor; codes are e4m3fn (RNE, saturating
+ * at +-448) of v/scale in fp32; scale = amax/448 (mode 0) or 2^ceil(log2(amax/448)) (mode 1); an all-zero
+ * block has scale 1.  1x128 blocks along the last axis / 128x128 blocks over the last two axes.
+ *   moe_quantize_act:    v [rows, cols] bf16 -> codes [rows, cols] u8, scales [rows, ceil(cols/128)] fp32
+ *   moe_quantize_weight: w [batch, rows, cols] bf16 -> codes u8, scales [batch, ceil(rows/128), ceil(cols/128)] */
+int32_t moe_quantize_act(const void* v, int64_t rows, int32_t cols, int32_t scale_mode, uint8_t* codes,
+                         float* scales, void* stream);
+int32_t moe_quantize_weight(const void* w, int32_t batch, int32_t rows, int32_t cols, int32_t scale_mode,
+                            uint8_t* codes, float* scales, void* stream);
+
+/* R1..R7: the whole forward.  X [T,H]; Wr [E,H]; bias [E] or NULL; Wg, Wu [E,F,H]; Wd [E,H,F];
+ * shared expert Wg_s, Wu_s [F_shared,H], Wd_s [H,F_shared] or NULL (iff F_shared == 0).
+ * Outputs Y [T,H], topk_idx [T,K], topk_w [T,K]; ctx receives what the backward needs. */
+int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
+                      const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                      const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
+                      void* stream);
+
+/* R8: the whole backward for L = <Y, dY>.  Weight gradients are overwritten, in the weights' type.
+ * Any of dWr / dWg / dWu / dWd (and the shared triple) may be NULL together with the others of its
+ * group to skip the weight-gradient GEMMs (dX is always produced). */
+int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const void* X, const void* Wr, const void* Wg,
+                      const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
+                      const void* ctx, void* dX, void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s,
+                      void* dWu_s, void* dWd_s, void* ws, void* stream);
+
+/* End-to-end step with HOST activations: copies X_host and dY_host [T,H] to the device buffers
+ * X_dev / dY_dev, runs moe_layer_fwd + moe_layer_bwd, copies Y and dX back to Y_host / dX_host, all on
+ * `stream` (host buffers should be pinned; returns without synchronising).  Weights, gradients, ctx,
+ * ws and the staging buffers X_dev, dY_dev, Y_dev, dX_dev are device memory. */
+int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const void* dY_host, void* Y_host,
+                            void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
+                            const void* Wr, const float* bias, const void* Wg, const void* Wu, const void* Wd,
+                            const void* Wg_s, const void* Wu_s, const void* Wd_s, void* dWr, void* dWg,
+                            void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, int32_t* topk_idx,
+                            float* topk_w, void* ctx, void* ws, void* stream);
+
+/* Read-only view of buffers inside ctx after moe_layer_fwd (for tests and tracing):
+ * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s"}.
+ * Writes the byte offset inside ctx and the byte length.  */
+int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
+/* Same for ws after moe_layer_bwd: {"dw","dz","dy","dgu","dXp"}. */
+int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
+
+/* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
+int64_t moe_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOE_B200_H */

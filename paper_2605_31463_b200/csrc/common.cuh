@@ -1,0 +1,115 @@
+// Shared host/device helpers of libmoe_b200 (sm_100a only).  Not part of the public ABI.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/moe_b200.h"
+
+namespace moe {
+
+extern long long g_launches;  // kernels launched since load (moe_launch_count)
+
+inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+// Every kernel launch in the library goes through this so that launches are counted and launch
+// errors become MOE_ERR_CUDA instead of being dropped.
+#define MOE_LAUNCH(kernel, grid, block, smem, stream, ...)                 \
+  do {                                                                     \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);            \
+    ++::moe::g_launches;                                                   \
+    if (cudaPeekAtLastError() != cudaSuccess) {                            \
+      cudaGetLastError();                                                  \
+      return MOE_ERR_CUDA;                                                 \
+    }                                                                      \
+  } while (0)
+
+#define MOE_CHECK(expr)                         \
+  do {                                          \
+    int32_t _s = (expr);                        \
+    if (_s != MOE_OK) return _s;                \
+  } while (0)
+
+#define MOE_CUDA(expr)                          \
+  do {                                          \
+    if ((expr) != cudaSuccess) {                \
+      cudaGetLastError();                       \
+      return MOE_ERR_CUDA;                      \
+    }                                           \
+  } while (0)
+
+inline int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+inline int64_t ceil_div(int64_t x, int64_t a) { return (x + a - 1) / a; }
+
+int32_t validate(const moe_config_t* c);
+inline int64_t padded_rows(const moe_config_t* c) {
+  int64_t tk = (int64_t)c->T * c->K;
+  if (c->row_align <= 1) return tk;
+  return round_up(tk + (int64_t)c->E * (c->row_align - 1), c->row_align);
+}
+inline size_t elem_bytes(const moe_config_t* c) { return c->dtype == 0 ? 4 : 2; }
+
+// ---- byte layout of ctx / ws ---------------------------------------------------------------
+struct CtxLayout {
+  size_t z, counts, offsets, p2f, f2p, mtile, Xp, gu, a, y, gu_s, a_s, y_s;
+  // fp8 (dtype 2): codes + scales of the quantised activations / weights kept for the backward
+  size_t Xq, Xq_s, Xpq, Xpq_s, aq, aq_s, Wgq, Wgq_s, Wuq, Wuq_s, Wdq, Wdq_s;
+  size_t asq, asq_s, Wgsq, Wgsq_s, Wusq, Wusq_s, Wdsq, Wdsq_s;
+  size_t total;
+};
+struct WsLayout {
+  size_t hist, tmp, dw, dz, dzp, dy, dgu, dXp, dgu_s, dXs, dYq, dYq_s, dyq, dyq_s, dguq, dguq_s, dgusq, dgusq_s;
+  size_t total;
+};
+CtxLayout ctx_layout(const moe_config_t* c);
+WsLayout ws_layout(const moe_config_t* c);
+
+constexpr int PERM_CHUNK = 1024;  // flat positions per counting-sort chunk (one CTA)
+
+// ---- internal entry points shared between translation units ---------------------------------------
+// permute.cu
+int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, int32_t* offsets, int32_t* p2f,
+                   int32_t* f2p, int32_t* mtile_expert, int32_t* hist, cudaStream_t s);
+int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, const int32_t* f2p, const int32_t* p2f,
+                    const int32_t* offsets, void* Xp, cudaStream_t s);
+int32_t combine(const moe_config_t* c, const void* y, const float* w, const int32_t* f2p, const void* add0,
+                const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s);
+int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const float* w, const int32_t* f2p,
+                    const int32_t* p2f, const int32_t* offsets, void* dy, float* dw, cudaStream_t s);
+// router.cu
+int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s);
+int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
+                   const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const void* Xp, float* dz,
+                   float* dzp, void* dWr, cudaStream_t s);
+// gemm_simt.cu: reference-free fallback GEMMs for fp32 (and any shape the tensor-core path rejects)
+//   mode 0: C[r,n]    = sum_k A[r,k] B[e][n,k]           (rows grouped by offsets)
+//   mode 1: dA[r,k]   = sum_n dC[r,n] B[e][n,k]
+//   mode 2: dB[e][n,k]= sum_{r in e} dC[r,n] A[r,k]
+int32_t simt_grouped_gemm(int mode, int dtype, int E, int N, int Kdim, const void* A, int lda, const void* B,
+                          const void* dC, int lddc, const int32_t* offsets, void* out, int ldo, cudaStream_t s);
+// gemm_tc.cu: tcgen05 grouped GEMMs (bf16)
+struct TcGemmArgs;
+int32_t tc_prepare_tiles(const int32_t* offsets, int E, int64_t rows_cap, int32_t* mtile_expert, cudaStream_t s);
+// elementwise.cu
+int32_t swiglu_fwd(int dtype, const void* gu, void* a, int64_t rows, int F, cudaStream_t s);
+int32_t swiglu_bwd(int dtype, const void* gu, const void* da, void* dgu, int64_t rows, int F, cudaStream_t s);
+
+// ---- device helpers --------------------------------------------------------------------------------
+__device__ __forceinline__ float bf16_to_f(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+template <typename T>
+__device__ __forceinline__ float to_f(T v);
+template <>
+__device__ __forceinline__ float to_f<float>(float v) { return v; }
+template <>
+__device__ __forceinline__ float to_f<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+template <typename T>
+__device__ __forceinline__ T from_f(float v);
+template <>
+__device__ __forceinline__ float from_f<float>(float v) { return v; }
+template <>
+__device__ __forceinline__ __nv_bfloat16 from_f<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+
+__device__ __forceinline__ float sigmoidf_acc(float x) { return 1.0f / (1.0f + expf(-x)); }
+
+}  // namespace moe

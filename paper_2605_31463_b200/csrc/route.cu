@@ -1,0 +1,190 @@
+// moe_route: top-k gating from fp32 logits.
+// One warp per token; lane l holds experts l, l+32, ... in registers; K rounds of warp arg-max by
+// shuffle with the (key desc, index asc) order, so ties go to the lower expert index.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace moe {
+namespace {
+
+constexpr unsigned FULL = 0xffffffffu;
+
+struct RouteParams {
+  int T, E, K, n_group, topk_group, score_fn, group_score, renorm, has_bias;
+  float routed_scale;
+};
+
+template <int VPT>
+__global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* __restrict__ logits,
+                                                    const float* __restrict__ bias, int32_t* __restrict__ topk_idx,
+                                                    float* __restrict__ topk_w) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (t >= p.T) return;
+  const float NEG = -INFINITY;
+  const float* zrow = logits + (size_t)t * p.E;
+
+  float z[VPT], key[VPT];
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) {
+    const int e = s * 32 + lane;
+    if (e < p.E) {
+      const float zv = zrow[e];
+      z[s] = zv;
+      float k;
+      if (p.score_fn == 0) {
+        k = zv;
+      } else {
+        // the (integer) selection is taken on fp32(sigmoid evaluated in fp64) + b, one fp32 add (R2)
+        k = (float)(1.0 / (1.0 + exp(-(double)zv)));
+      }
+      if (p.has_bias) k = k + bias[e];
+      key[s] = k;
+    } else {
+      z[s] = NEG;
+      key[s] = NEG;
+    }
+  }
+
+  // ---- R3 group-limited selection ----
+  if (p.n_group > 1 && p.topk_group < p.n_group) {
+    const int per = p.E / p.n_group;
+    float gscore = NEG;  // lane g holds the score of group g
+    for (int g = 0; g < p.n_group; ++g) {
+      float m1 = NEG, m2 = NEG;
+#pragma unroll
+      for (int s = 0; s < VPT; ++s) {
+        const int e = s * 32 + lane;
+        if (e < p.E && e / per == g) {
+          const float v = key[s];
+          if (v > m1) { m2 = m1; m1 = v; } else if (v > m2) { m2 = v; }
+        }
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        const float o1 = __shfl_xor_sync(FULL, m1, off);
+        const float o2 = __shfl_xor_sync(FULL, m2, off);
+        const float n1 = fmaxf(m1, o1);
+        const float n2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+        m1 = n1; m2 = n2;
+      }
+      const float sc = (p.group_score == 1 && per > 1) ? (m1 + m2) : m1;
+      if (lane == g) gscore = sc;
+    }
+    unsigned keep = 0;
+    for (int r = 0; r < p.topk_group; ++r) {
+      const bool avail = lane < p.n_group && !((keep >> lane) & 1u);
+      float v = avail ? gscore : NEG;
+      int gi = avail ? lane : 0x7fffffff;
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        const float ov = __shfl_xor_sync(FULL, v, off);
+        const int og = __shfl_xor_sync(FULL, gi, off);
+        const bool take = (og != 0x7fffffff) && (gi == 0x7fffffff || ov > v || (ov == v && og < gi));
+        if (take) { v = ov; gi = og; }
+      }
+      keep |= 1u << gi;
+    }
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      const int e = s * 32 + lane;
+      if (e < p.E && !((keep >> (e / per)) & 1u)) key[s] = NEG;
+    }
+  }
+
+  // ---- R4 top-k: K rounds of arg-max, ties -> lower expert index ----
+  int sel_e = 0;
+  float sel_z = 0.f;
+  unsigned taken = 0;  // bit s set: this lane's slot s was selected
+  for (int j = 0; j < p.K; ++j) {
+    float v = NEG;
+    int e = 0x7fffffff;
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      const int es = s * 32 + lane;
+      const bool ok = es < p.E && !((taken >> s) & 1u);
+      if (ok && (e == 0x7fffffff || key[s] > v)) { v = key[s]; e = es; }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const float ov = __shfl_xor_sync(FULL, v, off);
+      const int oe = __shfl_xor_sync(FULL, e, off);
+      const bool take = (oe != 0x7fffffff) && (e == 0x7fffffff || ov > v || (ov == v && oe < e));
+      if (take) { v = ov; e = oe; }
+    }
+    float zsel = 0.f;
+#pragma unroll
+    for (int s = 0; s < VPT; ++s)
+      if (s == (e >> 5)) zsel = z[s];
+    zsel = __shfl_sync(FULL, zsel, e & 31);
+    if (lane == (e & 31)) taken |= 1u << (e >> 5);
+    if (lane == j) { sel_e = e; sel_z = zsel; }
+  }
+
+  // ---- R5 gating weights (fp32) ----
+  const bool act = lane < p.K;
+  float wj;
+  if (p.score_fn == 0) {
+    float m, den;
+    if (p.renorm) {
+      m = act ? sel_z : NEG;
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, off));
+      den = act ? expf(sel_z - m) : 0.f;
+    } else {
+      m = NEG;
+#pragma unroll
+      for (int s = 0; s < VPT; ++s) m = fmaxf(m, z[s]);
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, off));
+      den = 0.f;
+#pragma unroll
+      for (int s = 0; s < VPT; ++s)
+        if (s * 32 + lane < p.E) den += expf(z[s] - m);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) den += __shfl_xor_sync(FULL, den, off);
+    wj = p.routed_scale * (expf(sel_z - m) / den);
+  } else {
+    const float sj = 1.0f / (1.0f + expf(-sel_z));
+    if (p.renorm) {
+      float sum = act ? sj : 0.f;
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(FULL, sum, off);
+      wj = p.routed_scale * (sj / (sum + 1e-20f));
+    } else {
+      wj = p.routed_scale * sj;
+    }
+  }
+  if (act) {
+    topk_idx[(size_t)t * p.K + lane] = sel_e;
+    topk_w[(size_t)t * p.K + lane] = wj;
+  }
+}
+
+}  // namespace
+
+}  // namespace moe
+
+extern "C" int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
+                             float* topk_w, void* stream) {
+  using namespace moe;
+  if (!cfg || !logits || !topk_idx || !topk_w) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
+  if (cfg->E > 1024 || cfg->K > 32 || cfg->n_group > 32) return MOE_ERR_UNSUPPORTED;
+  RouteParams p{cfg->T, cfg->E, cfg->K, cfg->n_group, cfg->topk_group, cfg->score_fn, cfg->group_score,
+                cfg->renorm, cfg->has_bias, cfg->routed_scale};
+  const int warps = 4;
+  dim3 grid((unsigned)ceil_div(cfg->T, warps)), block(warps * 32);
+  cudaStream_t s = as_stream(stream);
+  const int vpt = (int)ceil_div(cfg->E, 32);
+  if (vpt <= 1) MOE_LAUNCH(route_kernel<1>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  else if (vpt <= 2) MOE_LAUNCH(route_kernel<2>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  else if (vpt <= 4) MOE_LAUNCH(route_kernel<4>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  else if (vpt <= 8) MOE_LAUNCH(route_kernel<8>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  else if (vpt <= 16) MOE_LAUNCH(route_kernel<16>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  else MOE_LAUNCH(route_kernel<32>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  return MOE_OK;
+}
