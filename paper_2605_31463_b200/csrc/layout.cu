@@ -1,0 +1,179 @@
+// Config validation, ctx / ws byte layouts and the small query entry points of the C ABI.
+#include <string.h>
+
+#include "common.cuh"
+
+namespace moe {
+
+long long g_launches = 0;
+
+int32_t validate(const moe_config_t* c) {
+  if (!c) return MOE_ERR_INVALID_ARG;
+  if (c->T <= 0 || c->H <= 0 || c->E <= 0 || c->K <= 0 || c->F <= 0) return MOE_ERR_INVALID_ARG;
+  if (c->n_group < 1 || c->topk_group < 1 || c->topk_group > c->n_group) return MOE_ERR_INVALID_ARG;
+  if (c->score_fn < 0 || c->score_fn > 1 || c->group_score < 0 || c->group_score > 1) return MOE_ERR_INVALID_ARG;
+  if (c->dtype < 0 || c->dtype > 2 || c->fp8_scale_mode < 0 || c->fp8_scale_mode > 1) return MOE_ERR_INVALID_ARG;
+  if (c->row_align < 1 || c->F_shared < 0) return MOE_ERR_INVALID_ARG;
+  if (c->K > c->E) return MOE_ERR_UNSUPPORTED;
+  if (c->E % c->n_group != 0) return MOE_ERR_UNSUPPORTED;
+  if ((int64_t)c->K > (int64_t)c->topk_group * (c->E / c->n_group)) return MOE_ERR_UNSUPPORTED;
+  if ((int64_t)c->T * c->K >= (1ll << 31) || padded_rows(c) >= (1ll << 31)) return MOE_ERR_UNSUPPORTED;
+  const int a = c->dtype == 0 ? 4 : 8;  // 16-byte rows
+  if (c->H % a != 0 || c->F % a != 0 || c->F_shared % a != 0) return MOE_ERR_UNSUPPORTED;
+  if (c->dtype == 2 && (c->H % 128 != 0 || c->F % 128 != 0 || c->F_shared % 128 != 0)) return MOE_ERR_UNSUPPORTED;
+  return MOE_OK;
+}
+
+namespace {
+struct Carver {
+  size_t cur = 0;
+  size_t take(size_t bytes) {
+    const size_t at = cur;
+    cur += (bytes + 255) / 256 * 256;
+    return at;
+  }
+};
+}  // namespace
+
+CtxLayout ctx_layout(const moe_config_t* c) {
+  CtxLayout L;
+  memset(&L, 0, sizeof(L));
+  Carver k;
+  const size_t es = elem_bytes(c);
+  const size_t R = (size_t)padded_rows(c), T = c->T, H = c->H, F = c->F, E = c->E, Fs = c->F_shared;
+  L.z = k.take(T * E * 4);
+  L.counts = k.take(E * 4);
+  L.offsets = k.take((E + 1) * 4 + 16);  // + {0, T} for the shared expert's single group
+  L.p2f = k.take(R * 4);
+  L.f2p = k.take(T * c->K * 4);
+  L.mtile = k.take((R / 128 + 4) * 4);
+  L.Xp = k.take(R * H * es);
+  L.gu = k.take(R * 2 * F * es);
+  L.a = k.take(R * F * es);
+  L.y = k.take(R * H * es);
+  if (Fs) {
+    L.gu_s = k.take(T * 2 * Fs * es);
+    L.a_s = k.take(T * Fs * es);
+    L.y_s = k.take(T * H * es);
+  }
+  if (c->dtype == 2) {
+    L.Xq = k.take(T * H); L.Xq_s = k.take(T * (H / 128) * 4);
+    L.Xpq = k.take(R * H); L.Xpq_s = k.take(R * (H / 128) * 4);
+    L.aq = k.take(R * F); L.aq_s = k.take(R * (F / 128) * 4);
+    L.Wgq = k.take(E * F * H); L.Wgq_s = k.take(E * (F / 128) * (H / 128) * 4);
+    L.Wuq = k.take(E * F * H); L.Wuq_s = k.take(E * (F / 128) * (H / 128) * 4);
+    L.Wdq = k.take(E * H * F); L.Wdq_s = k.take(E * (H / 128) * (F / 128) * 4);
+    if (Fs) {
+      L.asq = k.take(T * Fs); L.asq_s = k.take(T * (Fs / 128) * 4);
+      L.Wgsq = k.take(Fs * H); L.Wgsq_s = k.take((Fs / 128) * (H / 128) * 4);
+      L.Wusq = k.take(Fs * H); L.Wusq_s = k.take((Fs / 128) * (H / 128) * 4);
+      L.Wdsq = k.take(H * Fs); L.Wdsq_s = k.take((H / 128) * (Fs / 128) * 4);
+    }
+  }
+  L.total = k.cur;
+  return L;
+}
+
+WsLayout ws_layout(const moe_config_t* c) {
+  WsLayout L;
+  memset(&L, 0, sizeof(L));
+  Carver k;
+  const size_t es = elem_bytes(c);
+  const size_t R = (size_t)padded_rows(c), T = c->T, H = c->H, F = c->F, E = c->E, Fs = c->F_shared;
+  const size_t nchunks = (T * c->K + PERM_CHUNK - 1) / PERM_CHUNK;
+  L.hist = k.take(nchunks * E * 4);
+  // tmp: M-tile table for stand-alone calls, or da [R,F] / da_s [T,Fs] on the CUDA-core path
+  size_t tmp = (R / 128 + 4) * 4;
+  if (R * F * es > tmp) tmp = R * F * es;
+  if (T * Fs * es > tmp) tmp = T * Fs * es;
+  L.tmp = k.take(tmp);
+  L.dw = k.take(T * c->K * 4);
+  L.dz = k.take(T * c->K * 4);
+  L.dzp = k.take(R * 4);
+  L.dy = k.take(R * H * es);
+  L.dgu = k.take(R * 2 * F * es);
+  L.dXp = k.take(R * H * es);
+  if (Fs) {
+    L.dgu_s = k.take(T * 2 * Fs * es);
+    L.dXs = k.take(T * H * es);
+  }
+  if (c->dtype == 2) {
+    L.dYq = k.take(T * H); L.dYq_s = k.take(T * (H / 128) * 4);
+    L.dyq = k.take(R * H); L.dyq_s = k.take(R * (H / 128) * 4);
+    L.dguq = k.take(R * 2 * F); L.dguq_s = k.take(R * (2 * F / 128) * 4);
+    if (Fs) { L.dgusq = k.take(T * 2 * Fs); L.dgusq_s = k.take(T * (2 * Fs / 128) * 4); }
+  }
+  L.total = k.cur;
+  return L;
+}
+
+}  // namespace moe
+
+using namespace moe;
+
+extern "C" const char* moe_status_string(int32_t status) {
+  switch (status) {
+    case MOE_OK: return "ok";
+    case MOE_ERR_INVALID_ARG: return "invalid argument";
+    case MOE_ERR_UNSUPPORTED: return "unsupported configuration";
+    case MOE_ERR_WORKSPACE: return "workspace error";
+    case MOE_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+extern "C" int32_t moe_version(void) { return 100; }
+
+extern "C" int64_t moe_launch_count(void) { return g_launches; }
+
+extern "C" int64_t moe_padded_rows(const moe_config_t* cfg) {
+  if (validate(cfg) != MOE_OK) return -1;
+  return padded_rows(cfg);
+}
+
+extern "C" int32_t moe_workspace_bytes(const moe_config_t* cfg, size_t* ws_bytes, size_t* ctx_bytes) {
+  MOE_CHECK(validate(cfg));
+  if (ws_bytes) *ws_bytes = ws_layout(cfg).total;
+  if (ctx_bytes) *ctx_bytes = ctx_layout(cfg).total;
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len) {
+  MOE_CHECK(validate(cfg));
+  if (!name || !byte_offset || !byte_len) return MOE_ERR_INVALID_ARG;
+  const CtxLayout L = ctx_layout(cfg);
+  const size_t es = elem_bytes(cfg);
+  const size_t R = (size_t)padded_rows(cfg), T = cfg->T, H = cfg->H, F = cfg->F, E = cfg->E, Fs = cfg->F_shared;
+  struct { const char* n; size_t off, len; } tab[] = {
+      {"z", L.z, T * E * 4}, {"counts", L.counts, E * 4}, {"offsets", L.offsets, (E + 1) * 4},
+      {"perm_to_flat", L.p2f, R * 4}, {"flat_to_perm", L.f2p, T * cfg->K * 4}, {"Xp", L.Xp, R * H * es},
+      {"gu", L.gu, R * 2 * F * es}, {"a", L.a, R * F * es}, {"y", L.y, R * H * es},
+      {"gu_s", L.gu_s, T * 2 * Fs * es}, {"a_s", L.a_s, T * Fs * es}, {"y_s", L.y_s, T * H * es}};
+  for (auto& t : tab)
+    if (strcmp(t.n, name) == 0) {
+      const size_t nl = strlen(name);
+      if (nl > 2 && strcmp(name + nl - 2, "_s") == 0 && !Fs) return MOE_ERR_INVALID_ARG;
+      *byte_offset = t.off;
+      *byte_len = t.len;
+      return MOE_OK;
+    }
+  return MOE_ERR_INVALID_ARG;
+}
+
+extern "C" int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len) {
+  MOE_CHECK(validate(cfg));
+  if (!name || !byte_offset || !byte_len) return MOE_ERR_INVALID_ARG;
+  const WsLayout L = ws_layout(cfg);
+  const size_t es = elem_bytes(cfg);
+  const size_t R = (size_t)padded_rows(cfg), T = cfg->T, H = cfg->H, F = cfg->F;
+  struct { const char* n; size_t off, len; } tab[] = {
+      {"dw", L.dw, T * cfg->K * 4}, {"dz", L.dz, T * cfg->K * 4}, {"dy", L.dy, R * H * es},
+      {"dgu", L.dgu, R * 2 * F * es}, {"dXp", L.dXp, R * H * es}};
+  for (auto& t : tab)
+    if (strcmp(t.n, name) == 0) {
+      *byte_offset = t.off;
+      *byte_len = t.len;
+      return MOE_OK;
+    }
+  return MOE_ERR_INVALID_ARG;
+}

@@ -1,0 +1,158 @@
+// Histogram + exclusive scan + stable counting sort of flat positions by expert, and the row movers
+// built on the resulting maps (SURVEY.md §8c R6, R7 combine, R8 combine-bwd).
+// No atomics anywhere: ranks come from warp match/ballot and per-chunk prefix tables, so the maps are
+// deterministic and bit-exact against the oracle's stable counting sort.
+#include "common.cuh"
+
+namespace moe {
+namespace {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int CHUNK_WARPS = 8;                                   // 256 threads per chunk CTA
+constexpr int CHUNK_ROUNDS = PERM_CHUNK / (CHUNK_WARPS * 32);    // rounds of 32 positions per warp
+
+// Per-warp running histogram over this warp's contiguous slice of the chunk.
+// rank[r] = number of earlier positions of the same expert inside this warp's slice.
+__device__ __forceinline__ void warp_rank(const int32_t* __restrict__ idx, int64_t TK, int64_t warp_base, int lane,
+                                          int32_t* wh, int (&ex)[CHUNK_ROUNDS], int (&rank)[CHUNK_ROUNDS]) {
+#pragma unroll
+  for (int r = 0; r < CHUNK_ROUNDS; ++r) {
+    const int64_t p = warp_base + r * 32 + lane;
+    const int e = (p < TK) ? idx[p] : -1;
+    ex[r] = e;
+    const unsigned m = __match_any_sync(FULL, e);
+    const int before = __popc(m & ((1u << lane) - 1u));
+    int base = 0;
+    if (e >= 0) base = wh[e];
+    rank[r] = base + before;
+    __syncwarp();
+    if (e >= 0 && before == 0) wh[e] = base + __popc(m);  // lowest lane of each match set updates
+    __syncwarp();
+  }
+}
+
+// Phase 1: hist[chunk][e] = number of positions of expert e in the chunk.
+__global__ void __launch_bounds__(CHUNK_WARPS * 32) hist_kernel(const int32_t* __restrict__ idx, int64_t TK, int E,
+                                                                 int32_t* __restrict__ hist) {
+  extern __shared__ int32_t wh[];  // [CHUNK_WARPS][E]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int i = threadIdx.x; i < CHUNK_WARPS * E; i += blockDim.x) wh[i] = 0;
+  __syncthreads();
+  int ex[CHUNK_ROUNDS], rank[CHUNK_ROUNDS];
+  const int64_t base = (int64_t)blockIdx.x * PERM_CHUNK + warp * (CHUNK_ROUNDS * 32);
+  warp_rank(idx, TK, base, lane, wh + warp * E, ex, rank);
+  __syncthreads();
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    int s = 0;
+#pragma unroll
+    for (int w = 0; w < CHUNK_WARPS; ++w) s += wh[w * E + e];
+    hist[(size_t)blockIdx.x * E + e] = s;
+  }
+}
+
+// Phase 2 (one CTA of 1024 threads): counts, aligned exclusive offsets, per-chunk bases (in place in
+// hist), and the M-tile -> expert table used by the tensor-core GEMMs (mtile[0] = number of 128-row
+// tiles, mtile[1 + i] = expert of tile i) when row_align is a multiple of 128.
+__global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, int nchunks, int E, int row_align,
+                                                    int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
+                                                    int32_t* __restrict__ mtile) {
+  __shared__ int32_t sh[1024];
+  __shared__ int32_t wsum[32];
+  const int e = threadIdx.x;
+  int cnt = 0;
+  if (e < E)
+    for (int c = 0; c < nchunks; ++c) cnt += hist[(size_t)c * E + e];
+  const int a = row_align < 1 ? 1 : row_align;
+  const int padded = (e < E) ? (cnt + a - 1) / a * a : 0;
+  // block-wide exclusive scan of `padded`
+  const int lane = e & 31, warp = e >> 5;
+  int v = padded;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const int o = __shfl_up_sync(FULL, v, off);
+    if (lane >= off) v += o;
+  }
+  if (lane == 31) wsum[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    int ws = wsum[lane];
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int o = __shfl_up_sync(FULL, ws, off);
+      if (lane >= off) ws += o;
+    }
+    wsum[lane] = ws;
+  }
+  __syncthreads();
+  const int incl = v + (warp > 0 ? wsum[warp - 1] : 0);
+  const int excl = incl - padded;
+  sh[e] = excl;
+  if (e < E) {
+    counts[e] = cnt;
+    offsets[e] = excl;
+    if (e == E - 1) offsets[E] = incl;
+    int run = excl;
+    for (int c = 0; c < nchunks; ++c) {
+      const int h = hist[(size_t)c * E + e];
+      hist[(size_t)c * E + e] = run;
+      run += h;
+    }
+    if (mtile != nullptr) {
+      for (int t = excl / 128; t < incl / 128; ++t) mtile[1 + t] = e;
+      if (e == E - 1) mtile[0] = incl / 128;
+    }
+  }
+}
+
+// Phase 3: scatter.  flat_to_perm[p] = base[chunk][e] + rank of p among the chunk's positions of e.
+__global__ void __launch_bounds__(CHUNK_WARPS * 32) scatter_kernel(const int32_t* __restrict__ idx, int64_t TK, int E,
+                                                                    const int32_t* __restrict__ chunk_base,
+                                                                    int32_t* __restrict__ p2f,
+                                                                    int32_t* __restrict__ f2p) {
+  extern __shared__ int32_t wh[];  // [CHUNK_WARPS][E]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int i = threadIdx.x; i < CHUNK_WARPS * E; i += blockDim.x) wh[i] = 0;
+  __syncthreads();
+  int ex[CHUNK_ROUNDS], rank[CHUNK_ROUNDS];
+  const int64_t base = (int64_t)blockIdx.x * PERM_CHUNK + warp * (CHUNK_ROUNDS * 32);
+  warp_rank(idx, TK, base, lane, wh + warp * E, ex, rank);
+  __syncthreads();
+  // turn per-warp totals into exclusive prefixes over warps, offset by the chunk base
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    int run = chunk_base[(size_t)blockIdx.x * E + e];
+#pragma unroll
+    for (int w = 0; w < CHUNK_WARPS; ++w) {
+      const int h = wh[w * E + e];
+      wh[w * E + e] = run;
+      run += h;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < CHUNK_ROUNDS; ++r) {
+    const int64_t p = base + r * 32 + lane;
+    if (ex[r] >= 0) {
+      const int row = wh[warp * E + ex[r]] + rank[r];
+      f2p[p] = row;
+      p2f[row] = (int32_t)p;
+    }
+  }
+}
+
+}  // namespace
+
+int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, int32_t* offsets, int32_t* p2f,
+                   int32_t* f2p, int32_t* mtile_expert, int32_t* hist, cudaStream_t s) {
+  const int64_t TK = (int64_t)c->T * c->K;
+  const int nchunks = (int)ceil_div(TK, PERM_CHUNK);
+  if (c->E > 1024) return MOE_ERR_UNSUPPORTED;
+  const size_t smem = (size_t)CHUNK_WARPS * c->E * sizeof(int32_t);
+  MOE_CUDA(cudaMemsetAsync(p2f, 0xFF, (size_t)padded_rows(c) * sizeof(int32_t), s));
+  MOE_LAUNCH(hist_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist);
+  int32_t* mt = (c->row_align % 128 == 0) ? mtile_expert : nullptr;
+  MOE_LAUNCH(scan_kernel, 1, 1024, 0, s, hist, nchunks, c->E, c->row_align, counts, offsets, mt);
+  MOE_LAUNCH(scatter_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist, p2f, f2p);
+  return MOE_OK;
+}
+
+}  // namespace moe

@@ -1,0 +1,245 @@
+// Row movers on the permutation maps: gather (moe_permute), weighted combine (moe_unpermute_combine,
+// also the dX reduction) and combine-backward.  SURVEY.md §8c R6/R7/R8.  All HBM-bound: one warp per
+// token, 16-byte vector accesses, each source row read once, fixed j order, fp32 accumulation.
+#include "common.cuh"
+
+namespace moe {
+namespace {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int ROW_WARPS = 8;
+
+__device__ __forceinline__ int4 ldg_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg_stream(int4* p, const int4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+               "r"(v.w));
+}
+
+// Xp[f2p[t*K+j]] = X[t] for j < K: token-major, the source row is read once and written K times.
+__global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __restrict__ X, int T, int K, int nvec,
+                                                                 const int32_t* __restrict__ f2p,
+                                                                 int4* __restrict__ Xp) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
+  if (t >= T) return;
+  const int4* src = X + (size_t)t * nvec;
+  const int32_t* rows = f2p + (size_t)t * K;
+  for (int v0 = 0; v0 < nvec; v0 += 128) {
+    int4 buf[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int v = v0 + u * 32 + lane;
+      if (v < nvec) buf[u] = ldg_stream(src + v);
+    }
+    for (int j = 0; j < K; ++j) {
+      int4* dst = Xp + (size_t)rows[j] * nvec;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int v = v0 + u * 32 + lane;
+        if (v < nvec) stg_stream(dst + v, buf[u]);
+      }
+    }
+  }
+}
+
+// Zero the padding rows (perm_to_flat[r] < 0) below offsets[E].
+__global__ void __launch_bounds__(ROW_WARPS * 32) zero_pad_kernel(const int32_t* __restrict__ p2f,
+                                                                   const int32_t* __restrict__ offsets, int E,
+                                                                   int nvec, int4* __restrict__ Xp) {
+  const int lane = threadIdx.x & 31;
+  const int rows = offsets[E];
+  const int wstride = gridDim.x * ROW_WARPS;
+  for (int r = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5); r < rows; r += wstride) {
+    if (p2f[r] >= 0) continue;
+    int4* dst = Xp + (size_t)r * nvec;
+    for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
+  }
+}
+
+template <typename T>
+struct Vec;
+template <>
+struct Vec<float> {
+  static constexpr int N = 4;
+  __device__ static void unpack(const int4& v, float (&f)[4]) {
+    f[0] = __int_as_float(v.x); f[1] = __int_as_float(v.y); f[2] = __int_as_float(v.z); f[3] = __int_as_float(v.w);
+  }
+  __device__ static int4 pack(const float (&f)[4]) {
+    return make_int4(__float_as_int(f[0]), __float_as_int(f[1]), __float_as_int(f[2]), __float_as_int(f[3]));
+  }
+};
+template <>
+struct Vec<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ static void unpack(const int4& v, float (&f)[8]) {
+    const int w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      f[2 * i] = __int_as_float(w[i] << 16);
+      f[2 * i + 1] = __int_as_float(w[i] & 0xffff0000);
+    }
+  }
+  __device__ static int4 pack(const float (&f)[8]) {
+    int w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const __nv_bfloat162 h = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
+      w[i] = *reinterpret_cast<const int*>(&h);
+    }
+    return make_int4(w[0], w[1], w[2], w[3]);
+  }
+};
+
+// Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
+template <typename T>
+__global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
+                                                                  const int32_t* __restrict__ f2p,
+                                                                  const int4* __restrict__ add0,
+                                                                  const float* __restrict__ dz,
+                                                                  const int32_t* __restrict__ idx,
+                                                                  const int4* __restrict__ Wr, int Tn, int K, int nvec,
+                                                                  int4* __restrict__ Y) {
+  constexpr int N = Vec<T>::N;
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
+  if (t >= Tn) return;
+  const int32_t* rows = f2p + (size_t)t * K;
+  for (int v = lane; v < nvec; v += 32) {
+    float acc[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) acc[i] = 0.f;
+    for (int j = 0; j < K; ++j) {
+      const float wj = w ? w[(size_t)t * K + j] : 1.0f;
+      float f[N];
+      Vec<T>::unpack(ldg_stream(y + (size_t)rows[j] * nvec + v), f);
+#pragma unroll
+      for (int i = 0; i < N; ++i) acc[i] = fmaf(wj, f[i], acc[i]);
+    }
+    if (add0) {
+      float f[N];
+      Vec<T>::unpack(ldg_stream(add0 + (size_t)t * nvec + v), f);
+#pragma unroll
+      for (int i = 0; i < N; ++i) acc[i] += f[i];
+    }
+    if (dz) {
+      for (int j = 0; j < K; ++j) {
+        const float d = dz[(size_t)t * K + j];
+        float f[N];
+        Vec<T>::unpack(__ldg(Wr + (size_t)idx[(size_t)t * K + j] * nvec + v), f);
+#pragma unroll
+        for (int i = 0; i < N; ++i) acc[i] = fmaf(d, f[i], acc[i]);
+      }
+    }
+    Y[(size_t)t * nvec + v] = Vec<T>::pack(acc);
+  }
+}
+
+// dy[f2p[t*K+j]] = w[t,j] * dY[t];   dw[t,j] = <dY[t], y[f2p[t*K+j]]>.
+template <typename T>
+__global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4* __restrict__ dY,
+                                                                      const int4* __restrict__ y,
+                                                                      const float* __restrict__ w,
+                                                                      const int32_t* __restrict__ f2p, int Tn, int K,
+                                                                      int nvec, int4* __restrict__ dy,
+                                                                      float* __restrict__ dw) {
+  constexpr int N = Vec<T>::N;
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
+  if (t >= Tn) return;
+  for (int j = 0; j < K; ++j) {
+    const int r = f2p[(size_t)t * K + j];
+    const float wj = w[(size_t)t * K + j];
+    float dot = 0.f;
+    for (int v = lane; v < nvec; v += 32) {
+      float g[N], f[N], o[N];
+      Vec<T>::unpack(__ldg(dY + (size_t)t * nvec + v), g);
+      Vec<T>::unpack(ldg_stream(y + (size_t)r * nvec + v), f);
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        dot = fmaf(g[i], f[i], dot);
+        o[i] = wj * g[i];
+      }
+      stg_stream(dy + (size_t)r * nvec + v, Vec<T>::pack(o));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(FULL, dot, off);
+    if (lane == 0) dw[(size_t)t * K + j] = dot;
+  }
+}
+
+}  // namespace
+
+int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, const int32_t* f2p, const int32_t* p2f,
+                    const int32_t* offsets, void* Xp, cudaStream_t s) {
+  if ((cols * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
+  const int nvec = (int)(cols * esz / 16);
+  MOE_LAUNCH(gather_kernel, (unsigned)ceil_div(c->T, ROW_WARPS), ROW_WARPS * 32, 0, s, (const int4*)X, c->T, c->K, nvec,
+             f2p, (int4*)Xp);
+  if (c->row_align > 1)
+    MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)Xp);
+  return MOE_OK;
+}
+
+int32_t combine(const moe_config_t* c, const void* y, const float* w, const int32_t* f2p, const void* add0,
+                const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s) {
+  const size_t esz = elem_bytes(c);
+  if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
+  const int nvec = (int)(c->H * esz / 16);
+  const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
+  if (c->dtype == 0)
+    MOE_LAUNCH(combine_kernel<float>, grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz, idx,
+               (const int4*)Wr, c->T, c->K, nvec, (int4*)Y);
+  else
+    MOE_LAUNCH(combine_kernel<__nv_bfloat16>, grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz,
+               idx, (const int4*)Wr, c->T, c->K, nvec, (int4*)Y);
+  return MOE_OK;
+}
+
+int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const float* w, const int32_t* f2p,
+                    const int32_t* p2f, const int32_t* offsets, void* dy, float* dw, cudaStream_t s) {
+  const size_t esz = elem_bytes(c);
+  if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
+  const int nvec = (int)(c->H * esz / 16);
+  const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
+  if (c->dtype == 0)
+    MOE_LAUNCH(combine_bwd_kernel<float>, grid, ROW_WARPS * 32, 0, s, (const int4*)dY, (const int4*)y, w, f2p, c->T,
+               c->K, nvec, (int4*)dy, dw);
+  else
+    MOE_LAUNCH(combine_bwd_kernel<__nv_bfloat16>, grid, ROW_WARPS * 32, 0, s, (const int4*)dY, (const int4*)y, w, f2p,
+               c->T, c->K, nvec, (int4*)dy, dw);
+  if (c->row_align > 1)
+    MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)dy);
+  return MOE_OK;
+}
+
+}  // namespace moe
+
+extern "C" int32_t moe_permute(const moe_config_t* cfg, const void* X, const int32_t* topk_idx, int32_t* counts,
+                               int32_t* offsets, int32_t* perm_to_flat, int32_t* flat_to_perm, void* Xp, void* ws,
+                               void* stream) {
+  using namespace moe;
+  if (!cfg || !topk_idx || !counts || !offsets || !perm_to_flat || !flat_to_perm || !ws) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  if (X && !Xp) return MOE_ERR_INVALID_ARG;
+  cudaStream_t s = as_stream(stream);
+  const WsLayout L = ws_layout(cfg);
+  int32_t* hist = reinterpret_cast<int32_t*>((char*)ws + L.hist);
+  int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + L.tmp);
+  MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, perm_to_flat, flat_to_perm, mtile, hist, s));
+  if (X) MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), flat_to_perm, perm_to_flat, offsets, Xp, s));
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_unpermute_combine(const moe_config_t* cfg, const void* y, const float* topk_w,
+                                         const int32_t* flat_to_perm, const void* shared_out, void* Y, void* stream) {
+  using namespace moe;
+  if (!cfg || !y || !topk_w || !flat_to_perm || !Y) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  return combine(cfg, y, topk_w, flat_to_perm, shared_out, nullptr, nullptr, nullptr, Y, as_stream(stream));
+}
