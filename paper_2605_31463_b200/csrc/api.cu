@@ -1,0 +1,74 @@
+// Public grouped-GEMM entry points and the host-buffer step (include/moe_b200.h).
+#include "common.cuh"
+
+namespace moe {
+int32_t tc_grouped_gemm_fwd(const moe_config_t* c, int N, int Kdim, const void* A, const void* B,
+                            const int32_t* offsets, void* C, int32_t* mtile_ws, cudaStream_t s);
+int32_t tc_grouped_gemm_bwd(const moe_config_t* c, int N, int Kdim, const void* dC, const void* A, const void* B,
+                            const int32_t* offsets, void* dA, void* dB, int32_t* mtile_ws, cudaStream_t s);
+int32_t fp8_grouped_gemm_fwd(const moe_config_t* c, int N, int Kdim, const void* A, const void* B,
+                             const int32_t* offsets, void* C, const float* a_scales, const float* b_scales,
+                             int32_t* mtile_ws, cudaStream_t s);
+}  // namespace moe
+
+using namespace moe;
+
+extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int32_t Kdim, const void* A,
+                                        const void* B, const int32_t* offsets, void* C, const void* a_scales,
+                                        const void* b_scales, void* ws, void* stream) {
+  if (!cfg || !A || !B || !offsets || !C || !ws || N <= 0 || Kdim <= 0) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  cudaStream_t s = as_stream(stream);
+  int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + ws_layout(cfg).tmp);
+  if (cfg->dtype == 2) {
+    if (!a_scales || !b_scales) return MOE_ERR_INVALID_ARG;
+    return fp8_grouped_gemm_fwd(cfg, N, Kdim, A, B, offsets, C, (const float*)a_scales, (const float*)b_scales, mtile,
+                                s);
+  }
+  if (cfg->dtype == 1) {
+    const int32_t st = tc_grouped_gemm_fwd(cfg, N, Kdim, A, B, offsets, C, mtile, s);
+    if (st != MOE_ERR_UNSUPPORTED) return st;
+  }
+  return simt_grouped_gemm(0, cfg->dtype, cfg->E, N, Kdim, A, Kdim, B, nullptr, 0, offsets, C, N, padded_rows(cfg), 0,
+                           s);
+}
+
+extern "C" int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int32_t Kdim, const void* dC,
+                                        const void* A, const void* B, const int32_t* offsets, void* dA, void* dB,
+                                        void* ws, void* stream) {
+  if (!cfg || !dC || !offsets || !ws || N <= 0 || Kdim <= 0) return MOE_ERR_INVALID_ARG;
+  if ((dA && !B) || (dB && !A)) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;
+  cudaStream_t s = as_stream(stream);
+  int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + ws_layout(cfg).tmp);
+  if (cfg->dtype == 1) {
+    const int32_t st = tc_grouped_gemm_bwd(cfg, N, Kdim, dC, A, B, offsets, dA, dB, mtile, s);
+    if (st != MOE_ERR_UNSUPPORTED) return st;
+  }
+  const int64_t R = padded_rows(cfg);
+  if (dA) MOE_CHECK(simt_grouped_gemm(1, cfg->dtype, cfg->E, N, Kdim, nullptr, 0, B, dC, N, offsets, dA, Kdim, R, 0, s));
+  if (dB) MOE_CHECK(simt_grouped_gemm(2, cfg->dtype, cfg->E, N, Kdim, A, Kdim, nullptr, dC, N, offsets, dB, 0, R, 0, s));
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const void* dY_host, void* Y_host,
+                                       void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
+                                       const void* Wr, const float* bias, const void* Wg, const void* Wu,
+                                       const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s, void* dWr,
+                                       void* dWg, void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s,
+                                       int32_t* topk_idx, float* topk_w, void* ctx, void* ws, void* stream) {
+  if (!cfg || !X_host || !dY_host || !Y_host || !dX_host || !X_dev || !dY_dev || !Y_dev || !dX_dev)
+    return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  cudaStream_t s = as_stream(stream);
+  const size_t bytes = (size_t)cfg->T * cfg->H * elem_bytes(cfg);
+  MOE_CUDA(cudaMemcpyAsync(X_dev, X_host, bytes, cudaMemcpyHostToDevice, s));
+  MOE_CUDA(cudaMemcpyAsync(dY_dev, dY_host, bytes, cudaMemcpyHostToDevice, s));
+  MOE_CHECK(moe_layer_fwd(cfg, X_dev, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, Y_dev, topk_idx, topk_w, ctx, ws, stream));
+  MOE_CHECK(moe_layer_bwd(cfg, dY_dev, X_dev, Wr, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, dX_dev, dWr, dWg, dWu, dWd, dWg_s,
+                          dWu_s, dWd_s, ws, stream));
+  MOE_CUDA(cudaMemcpyAsync(Y_host, Y_dev, bytes, cudaMemcpyDeviceToHost, s));
+  MOE_CUDA(cudaMemcpyAsync(dX_host, dX_dev, bytes, cudaMemcpyDeviceToHost, s));
+  return MOE_OK;
+}

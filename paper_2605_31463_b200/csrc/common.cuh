@@ -51,7 +51,7 @@ inline size_t elem_bytes(const moe_config_t* c) { return c->dtype == 0 ? 4 : 2; 
 
 // ---- byte layout of ctx / ws ---------------------------------------------------------------
 struct CtxLayout {
-  size_t z, counts, offsets, p2f, f2p, mtile, Xp, gu, a, y, gu_s, a_s, y_s;
+  size_t z, idx, w, counts, offsets, p2f, f2p, mtile, Xp, gu, a, y, gu_s, a_s, y_s;
   // fp8 (dtype 2): codes + scales of the quantised activations / weights kept for the backward
   size_t Xq, Xq_s, Xpq, Xpq_s, aq, aq_s, Wgq, Wgq_s, Wuq, Wuq_s, Wdq, Wdq_s;
   size_t asq, asq_s, Wgsq, Wgsq_s, Wusq, Wusq_s, Wdsq, Wdsq_s;
@@ -86,7 +86,8 @@ int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, co
 //   mode 1: dA[r,k]   = sum_n dC[r,n] B[e][n,k]
 //   mode 2: dB[e][n,k]= sum_{r in e} dC[r,n] A[r,k]
 int32_t simt_grouped_gemm(int mode, int dtype, int E, int N, int Kdim, const void* A, int lda, const void* B,
-                          const void* dC, int lddc, const int32_t* offsets, void* out, int ldo, cudaStream_t s);
+                          const void* dC, int lddc, const int32_t* offsets, void* out, int ldo, int64_t rows_cap,
+                          int accumulate, cudaStream_t s);
 // gemm_tc.cu: tcgen05 grouped GEMMs (bf16)
 struct TcGemmArgs;
 int32_t tc_prepare_tiles(const int32_t* offsets, int E, int64_t rows_cap, int32_t* mtile_expert, cudaStream_t s);

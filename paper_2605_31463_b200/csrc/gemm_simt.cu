@@ -18,6 +18,7 @@ struct SimtArgs {
   void* out;
   const int32_t* offsets;
   int max_row_tiles;  // grid.x for modes 0/1
+  int accumulate;     // 1: out += result (second half of a split contraction)
 };
 
 template <typename T>
@@ -116,7 +117,7 @@ __global__ void __launch_bounds__(256) simt_kernel(SimtArgs p) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const int n = n0 + tx * 4 + j;
-      if (n < Ncols) out[m * ldo + n] = from_f<T>(acc[i][j]);
+      if (n < Ncols) out[m * ldo + n] = from_f<T>(acc[i][j] + (p.accumulate ? to_f(out[m * ldo + n]) : 0.f));
     }
   }
 }
@@ -125,8 +126,8 @@ __global__ void __launch_bounds__(256) simt_kernel(SimtArgs p) {
 
 int32_t simt_grouped_gemm(int mode, int dtype, int E, int N, int Kdim, const void* A, int lda, const void* B,
                           const void* dC, int lddc, const int32_t* offsets, void* out, int ldo, int64_t rows_cap,
-                          cudaStream_t s) {
-  SimtArgs p{mode, E, N, Kdim, lda, lddc, ldo, A, B, dC, out, offsets, 0};
+                          int accumulate, cudaStream_t s) {
+  SimtArgs p{mode, E, N, Kdim, lda, lddc, ldo, A, B, dC, out, offsets, 0, accumulate};
   dim3 grid;
   if (mode == 2) {
     grid = dim3((unsigned)ceil_div(N, TS), (unsigned)ceil_div(Kdim, TS), (unsigned)E);

@@ -1,0 +1,178 @@
+// moe_layer_fwd / moe_layer_bwd: composition of the hot path (SURVEY.md §3 call stack, §8c R1..R8),
+// plus the public grouped-GEMM entry points.  Single stream, no host synchronisation anywhere:
+// per-expert counts stay on the device.
+#include "common.cuh"
+
+namespace moe {
+
+// One SwiGLU FFN over grouped rows: the routed experts (E groups from the permutation) or the
+// shared expert (one group holding every token).
+struct FfnGroup {
+  int dtype, E, H, F;
+  int64_t rows_cap;        // upper bound on rows (buffer height)
+  const int32_t* offsets;  // [E+1] device
+  const int32_t* counts;   // [E] device or nullptr (then offsets differences are used)
+  const int32_t* mtile;    // M-tile -> expert table (tensor-core path) or nullptr
+  int row_align;
+};
+
+int32_t tc_ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* Wu, const void* Wd, void* gu,
+                   void* a, void* y, cudaStream_t s);
+int32_t tc_ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* gu, const void* a, const void* Wg,
+                   const void* Wu, const void* Wd, void* dgu, void* dXp, void* dWg, void* dWu, void* dWd,
+                   cudaStream_t s);
+
+namespace {
+
+__global__ void set2_kernel(int32_t* p, int32_t a, int32_t b) {
+  p[0] = a;
+  p[1] = b;
+}
+
+int32_t ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* Wu, const void* Wd, void* gu, void* a,
+                void* y, cudaStream_t s) {
+  if (g.dtype != 0) {
+    const int32_t st = tc_ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s);
+    if (st != MOE_ERR_UNSUPPORTED) return st;
+  }
+  const size_t es = g.dtype == 0 ? 4 : 2;
+  MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.F, g.H, Xp, g.H, Wg, nullptr, 0, g.offsets, gu, 2 * g.F, g.rows_cap, 0, s));
+  MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.F, g.H, Xp, g.H, Wu, nullptr, 0, g.offsets, (char*)gu + g.F * es,
+                              2 * g.F, g.rows_cap, 0, s));
+  MOE_CHECK(swiglu_fwd(g.dtype, gu, a, g.rows_cap, g.F, s));
+  MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.H, g.F, a, g.F, Wd, nullptr, 0, g.offsets, y, g.H, g.rows_cap, 0, s));
+  return MOE_OK;
+}
+
+// dy [rows,H] -> dgu, dXp and (optionally) dWg, dWu, dWd.  da_tmp [rows,F] is scratch (CUDA-core path only).
+int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* gu, const void* a, const void* Wg,
+                const void* Wu, const void* Wd, void* da_tmp, void* dgu, void* dXp, void* dWg, void* dWu, void* dWd,
+                cudaStream_t s) {
+  if (g.dtype != 0) {
+    const int32_t st = tc_ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, dgu, dXp, dWg, dWu, dWd, s);
+    if (st != MOE_ERR_UNSUPPORTED) return st;
+  }
+  const size_t es = g.dtype == 0 ? 4 : 2;
+  const void* dgu_u = (const char*)dgu + g.F * es;
+  // da = dy Wd[e]            (B = Wd [E,H,F]: N = H, Kdim = F)
+  MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.H, g.F, nullptr, 0, Wd, dy, g.H, g.offsets, da_tmp, g.F, g.rows_cap, 0, s));
+  MOE_CHECK(swiglu_bwd(g.dtype, gu, da_tmp, dgu, g.rows_cap, g.F, s));
+  // dXp = dg Wg[e] + du Wu[e]  (B = Wg [E,F,H]: N = F, Kdim = H)
+  MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wg, dgu, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 0, s));
+  MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wu, dgu_u, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 1, s));
+  if (dWd) {
+    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.H, g.F, a, g.F, nullptr, dy, g.H, g.offsets, dWd, 0, g.rows_cap, 0, s));
+    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu, 2 * g.F, g.offsets, dWg, 0, g.rows_cap, 0, s));
+    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu_u, 2 * g.F, g.offsets, dWu, 0, g.rows_cap, 0, s));
+  }
+  return MOE_OK;
+}
+
+template <typename T>
+T* at(const void* base, size_t off) {
+  return reinterpret_cast<T*>((char*)base + off);
+}
+
+}  // namespace
+}  // namespace moe
+
+using namespace moe;
+
+extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
+                                 const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                                 const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
+                                 void* stream) {
+  if (!cfg || !X || !Wr || !Wg || !Wu || !Wd || !Y || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
+  const bool shared = cfg->F_shared > 0;
+  if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;  // fp8 layer path: see layer_fp8.cu when present
+  cudaStream_t s = as_stream(stream);
+  const CtxLayout C = ctx_layout(cfg);
+  const WsLayout W = ws_layout(cfg);
+  float* z = at<float>(ctx, C.z);
+  int32_t* counts = at<int32_t>(ctx, C.counts);
+  int32_t* offsets = at<int32_t>(ctx, C.offsets);
+  int32_t* p2f = at<int32_t>(ctx, C.p2f);
+  int32_t* f2p = at<int32_t>(ctx, C.f2p);
+  int32_t* mtile = at<int32_t>(ctx, C.mtile);
+  void* Xp = at<char>(ctx, C.Xp);
+  void* gu = at<char>(ctx, C.gu);
+  void* a = at<char>(ctx, C.a);
+  void* y = at<char>(ctx, C.y);
+
+  MOE_CHECK(router_logits(cfg, X, Wr, z, s));                                              // R1
+  MOE_CHECK(moe_route(cfg, z, bias, topk_idx, topk_w, stream));                            // R2..R5
+  MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.idx), topk_idx, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
+  MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.w), topk_w, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
+  MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, p2f, f2p, mtile, at<int32_t>(ws, W.hist), s));  // R6
+  MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, Xp, s));
+  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
+             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align};
+  MOE_CHECK(ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s));                                      // R7
+  const void* shared_out = nullptr;
+  if (shared) {
+    int32_t* off_s = offsets + cfg->E + 1;
+    MOE_LAUNCH(set2_kernel, 1, 1, 0, s, off_s, 0, cfg->T);
+    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1};
+    MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
+    shared_out = at<char>(ctx, C.y_s);
+  }
+  MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, Y, s));    // R7 combine
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const void* X, const void* Wr,
+                                 const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                                 const void* Wd_s, const void* ctx, void* dX, void* dWr, void* dWg, void* dWu,
+                                 void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, void* ws, void* stream) {
+  if (!cfg || !dY || !X || !Wr || !Wg || !Wu || !Wd || !ctx || !dX || !ws) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  const bool shared = cfg->F_shared > 0;
+  if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  const bool wgrad = dWg || dWu || dWd;
+  if (wgrad && !(dWg && dWu && dWd)) return MOE_ERR_INVALID_ARG;
+  const bool wgrad_s = dWg_s || dWu_s || dWd_s;
+  if (wgrad_s && !(shared && dWg_s && dWu_s && dWd_s)) return MOE_ERR_INVALID_ARG;
+  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;
+  cudaStream_t s = as_stream(stream);
+  const CtxLayout C = ctx_layout(cfg);
+  const WsLayout W = ws_layout(cfg);
+  const float* z = at<float>(ctx, C.z);
+  const int32_t* counts = at<int32_t>(ctx, C.counts);
+  const int32_t* offsets = at<int32_t>(ctx, C.offsets);
+  const int32_t* p2f = at<int32_t>(ctx, C.p2f);
+  const int32_t* f2p = at<int32_t>(ctx, C.f2p);
+  const int32_t* mtile = at<int32_t>(ctx, C.mtile);
+  const int32_t* idx = at<int32_t>(ctx, C.idx);
+  const float* w = at<float>(ctx, C.w);
+  const void* Xp = at<char>(ctx, C.Xp);
+  const void* gu = at<char>(ctx, C.gu);
+  const void* a = at<char>(ctx, C.a);
+  const void* y = at<char>(ctx, C.y);
+  float* dw = at<float>(ws, W.dw);
+  float* dz = at<float>(ws, W.dz);
+  float* dzp = at<float>(ws, W.dzp);
+  void* dy = at<char>(ws, W.dy);
+  void* dgu = at<char>(ws, W.dgu);
+  void* dXp = at<char>(ws, W.dXp);
+  void* tmp = at<char>(ws, W.tmp);
+
+  MOE_CHECK(combine_bwd(cfg, dY, y, w, f2p, p2f, offsets, dy, dw, s));                     // R8 combine-bwd
+  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
+             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align};
+  MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));       // R8 expert FFN
+  MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, Xp, dz, dzp, dWr, s));    // R8 router
+  const void* dXs = nullptr;
+  if (shared) {
+    const int32_t* off_s = offsets + cfg->E + 1;
+    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1};
+    MOE_CHECK(ffn_bwd(gs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), Wg_s, Wu_s, Wd_s, tmp,
+                      at<char>(ws, W.dgu_s), at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
+    dXs = at<char>(ws, W.dXs);
+  }
+  // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]
+  MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, dz, idx, Wr, dX, s));
+  return MOE_OK;
+}

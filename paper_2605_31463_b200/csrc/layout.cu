@@ -42,6 +42,8 @@ CtxLayout ctx_layout(const moe_config_t* c) {
   const size_t es = elem_bytes(c);
   const size_t R = (size_t)padded_rows(c), T = c->T, H = c->H, F = c->F, E = c->E, Fs = c->F_shared;
   L.z = k.take(T * E * 4);
+  L.idx = k.take(T * c->K * 4);
+  L.w = k.take(T * c->K * 4);
   L.counts = k.take(E * 4);
   L.offsets = k.take((E + 1) * 4 + 16);  // + {0, T} for the shared expert's single group
   L.p2f = k.take(R * 4);
