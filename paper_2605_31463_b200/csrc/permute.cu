@@ -56,7 +56,6 @@ __global__ void __launch_bounds__(CHUNK_WARPS * 32) hist_kernel(const int32_t* _
 __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, int nchunks, int E, int row_align,
                                                     int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
                                                     int32_t* __restrict__ mtile) {
-  __shared__ int32_t sh[1024];
   __shared__ int32_t wsum[32];
   const int e = threadIdx.x;
   int cnt = 0;
@@ -86,7 +85,6 @@ __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, 
   __syncthreads();
   const int incl = v + (warp > 0 ? wsum[warp - 1] : 0);
   const int excl = incl - padded;
-  sh[e] = excl;
   if (e < E) {
     counts[e] = cnt;
     offsets[e] = excl;
