@@ -165,6 +165,15 @@ int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size_t* byte_of
 /* Same for ws after moe_layer_bwd: {"dw","dz","dy","dgu","dXp"}. */
 int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
 
+/* Stage timing for bench.py: while enabled, moe_layer_fwd / moe_layer_bwd record a CUDA event on
+ * their stream after every stage; moe_profile_stage_ms synchronises on those events and returns the summed
+ * device time and the number of recorded segments of one stage since the last moe_profile_enable call.  Stages:
+ * "router_gemm","route","maps","permute","gemm1_swiglu","gemm2","combine","combine_bwd","dgrad_down_swiglu",
+ * "dgrad_gateup","wgrad","router_bwd","dx_combine","shared_fwd","shared_bwd","quant".  Host-side state, not
+ * thread-safe; at most 8192 marks are kept between two enable calls. */
+int32_t moe_profile_enable(int32_t on);
+int32_t moe_profile_stage_ms(const char* stage, double* total_ms, int64_t* segments);
+
 /* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
 int64_t moe_launch_count(void);
 

@@ -64,6 +64,8 @@ _SIGNATURES = {
     "moe_layer_step_host": (_I32, [_CFG] + [_P] * 28),
     "moe_ctx_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
     "moe_ws_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
+    "moe_profile_enable": (_I32, [_I32]),
+    "moe_profile_stage_ms": (_I32, [C.c_char_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
 }
 EXPORTS = sorted(_SIGNATURES)
 
@@ -117,6 +119,20 @@ def moe_version() -> int:
 
 def moe_launch_count() -> int:
     return lib().moe_launch_count()
+
+
+STAGES = ["router_gemm", "route", "maps", "permute", "gemm1_swiglu", "gemm2", "combine", "combine_bwd",
+          "dgrad_down_swiglu", "dgrad_gateup", "wgrad", "router_bwd", "dx_combine", "shared_fwd", "shared_bwd", "quant"]
+
+
+def moe_profile_enable(on: bool):
+    _check(lib().moe_profile_enable(1 if on else 0), "moe_profile_enable")
+
+
+def moe_profile_stage_ms(stage: str):
+    ms, n = C.c_double(0), C.c_int64(0)
+    _check(lib().moe_profile_stage_ms(stage.encode(), C.byref(ms), C.byref(n)), "moe_profile_stage_ms")
+    return ms.value, n.value
 
 
 def moe_padded_rows(cfg) -> int:

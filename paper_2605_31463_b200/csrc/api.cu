@@ -1,15 +1,7 @@
 // Public grouped-GEMM entry points and the host-buffer step (include/moe_b200.h).
-#include "common.cuh"
+#include <string.h>
 
-namespace moe {
-int32_t tc_grouped_gemm_fwd(const moe_config_t* c, int N, int Kdim, const void* A, const void* B,
-                            const int32_t* offsets, void* C, int32_t* mtile_ws, cudaStream_t s);
-int32_t tc_grouped_gemm_bwd(const moe_config_t* c, int N, int Kdim, const void* dC, const void* A, const void* B,
-                            const int32_t* offsets, void* dA, void* dB, int32_t* mtile_ws, cudaStream_t s);
-int32_t fp8_grouped_gemm_fwd(const moe_config_t* c, int N, int Kdim, const void* A, const void* B,
-                             const int32_t* offsets, void* C, const float* a_scales, const float* b_scales,
-                             int32_t* mtile_ws, cudaStream_t s);
-}  // namespace moe
+#include "gemm_tc.cuh"
 
 using namespace moe;
 
@@ -20,13 +12,15 @@ extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int3
   MOE_CHECK(validate(cfg));
   cudaStream_t s = as_stream(stream);
   int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + ws_layout(cfg).tmp);
-  if (cfg->dtype == 2) {
-    if (!a_scales || !b_scales) return MOE_ERR_INVALID_ARG;
-    return fp8_grouped_gemm_fwd(cfg, N, Kdim, A, B, offsets, C, (const float*)a_scales, (const float*)b_scales, mtile,
-                                s);
-  }
-  if (cfg->dtype == 1) {
-    const int32_t st = tc_grouped_gemm_fwd(cfg, N, Kdim, A, B, offsets, C, mtile, s);
+  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;   // stand-alone fp8 GEMM: see fp8.cu
+  (void)a_scales; (void)b_scales;
+  if (cfg->dtype == 1 && cfg->row_align % 128 == 0 && Kdim % 64 == 0 && N % 8 == 0) {
+    MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
+    TcCall c;
+    memset(&c, 0, sizeof(c));
+    c.mode = TC_FWD; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    c.A = A; c.lda = Kdim; c.B0 = B; c.b_rows = N; c.b_cols = Kdim; c.N = N; c.Kd = Kdim; c.out0 = C; c.ld0 = N;
+    const int32_t st = tc_gemm(c, s);
     if (st != MOE_ERR_UNSUPPORTED) return st;
   }
   return simt_grouped_gemm(0, cfg->dtype, cfg->E, N, Kdim, A, Kdim, B, nullptr, 0, offsets, C, N, padded_rows(cfg), 0,
@@ -42,9 +36,22 @@ extern "C" int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int3
   if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;
   cudaStream_t s = as_stream(stream);
   int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + ws_layout(cfg).tmp);
-  if (cfg->dtype == 1) {
-    const int32_t st = tc_grouped_gemm_bwd(cfg, N, Kdim, dC, A, B, offsets, dA, dB, mtile, s);
-    if (st != MOE_ERR_UNSUPPORTED) return st;
+  if (cfg->dtype == 1 && cfg->row_align % 128 == 0 && N % 64 == 0 && Kdim % 8 == 0) {
+    MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
+    TcCall c;
+    memset(&c, 0, sizeof(c));
+    c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    if (dA) {   // dA = dC B[e]: contraction over B's rows
+      c.mode = TC_DGRAD; c.A = dC; c.lda = N; c.B0 = B; c.B1 = nullptr; c.b_rows = N; c.b_cols = Kdim; c.N = Kdim;
+      c.out0 = dA; c.ld0 = Kdim;
+      MOE_CHECK(tc_gemm(c, s));
+    }
+    if (dB) {   // dB[e] = dC_e^T A_e
+      c.mode = TC_WGRAD; c.A = dC; c.lda = N; c.a_col0 = 0; c.M = N; c.A2 = A; c.lda2 = Kdim; c.N = Kdim;
+      c.out0 = dB; c.ld0 = Kdim;
+      MOE_CHECK(tc_gemm(c, s));
+    }
+    return MOE_OK;
   }
   const int64_t R = padded_rows(cfg);
   if (dA) MOE_CHECK(simt_grouped_gemm(1, cfg->dtype, cfg->E, N, Kdim, nullptr, 0, B, dC, N, offsets, dA, Kdim, R, 0, s));

@@ -10,6 +10,14 @@ namespace moe {
 
 extern long long g_launches;  // kernels launched since load (moe_launch_count)
 
+// Stage timing (moe_profile_*): a mark attributes the stream time since the previous mark to `stage`.
+enum Stage { ST_BEGIN = 0, ST_ROUTER_GEMM, ST_ROUTE, ST_MAPS, ST_PERMUTE, ST_GEMM1_SWIGLU, ST_GEMM2, ST_COMBINE,
+             ST_COMBINE_BWD, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD, ST_ROUTER_BWD, ST_DX_COMBINE,
+             ST_SHARED_FWD, ST_SHARED_BWD, ST_QUANT, ST_COUNT };
+extern int g_prof_on;
+void prof_mark_impl(int stage, cudaStream_t s);
+inline void prof_mark(int stage, cudaStream_t s) { if (g_prof_on) prof_mark_impl(stage, s); }
+
 inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
 
 // Every kernel launch in the library goes through this so that launches are counted and launch

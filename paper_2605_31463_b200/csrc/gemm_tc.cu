@@ -1,24 +1,593 @@
-// tcgen05 grouped GEMMs (placeholder until the kernels land): every entry reports UNSUPPORTED so the
-// callers take the CUDA-core path.
-#include "common.cuh"
+// tcgen05 / TMEM / TMA grouped GEMMs for sm_100a (bf16 in, fp32 accumulate in tensor memory, bf16 out).
+//
+// One persistent, warp-specialised kernel template serves every expert GEMM of the layer (SURVEY.md §8a
+// a5, a6, a9..a12): warp 0 = TMA producer, warp 1 = MMA issuer (one elected thread, tcgen05.mma
+// cta_group::1, M=128 x N=256 x K=16 per instruction), warps 2..5 = epilogue (tcgen05.ld from a
+// double-buffered 2 x 256-column TMEM accumulator).  Operands are staged by TMA into 128-byte-swizzled
+// shared memory, 4 stages of (128 x 64 A tile + 256 x 64 B tile) = 192 KB.  The tile schedule is
+// computed on the device from the per-expert row offsets (shapes are data dependent; the
+// counts never visit the host): a 128-row M-tile belongs to exactly one expert because expert groups
+// start at multiples of 128 rows.  SwiGLU forward / backward are fused into the epilogues.
+// Both K-major and MN-major shared-memory operand layouts are used, so the dgrad (weights read
+// "transposed") and wgrad (both operands contracted over rows) need no transposed copies in HBM.
+#include <cuda.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "gemm_tc.cuh"
 
 namespace moe {
-struct FfnGroup;
-int32_t tc_ffn_fwd(const FfnGroup&, const void*, const void*, const void*, const void*, void*, void*, void*,
-                   cudaStream_t) { return MOE_ERR_UNSUPPORTED; }
-int32_t tc_ffn_bwd(const FfnGroup&, const void*, const void*, const void*, const void*, const void*, const void*,
-                   const void*, void*, void*, void*, void*, void*, cudaStream_t) { return MOE_ERR_UNSUPPORTED; }
-int32_t tc_grouped_gemm_fwd(const moe_config_t*, int, int, const void*, const void*, const int32_t*, void*, int32_t*,
-                            cudaStream_t) { return MOE_ERR_UNSUPPORTED; }
-int32_t tc_grouped_gemm_bwd(const moe_config_t*, int, int, const void*, const void*, const void*, const int32_t*,
-                            void*, void*, int32_t*, cudaStream_t) { return MOE_ERR_UNSUPPORTED; }
-int32_t fp8_grouped_gemm_fwd(const moe_config_t*, int, int, const void*, const void*, const int32_t*, void*,
-                             const float*, const float*, int32_t*, cudaStream_t) { return MOE_ERR_UNSUPPORTED; }
-}  // namespace moe
+namespace {
 
-extern "C" int32_t moe_quantize_act(const void*, int64_t, int32_t, int32_t, uint8_t*, float*, void*) {
-  return MOE_ERR_UNSUPPORTED;
+constexpr int BM = 128;      // tile rows  (UMMA M)
+constexpr int BN = 256;      // tile cols  (UMMA N)
+constexpr int BK = 64;       // k-block: 64 bf16 = 128 bytes = one swizzle span
+constexpr int UK = 16;       // UMMA K for 16-bit operands
+constexpr int STAGES = 4;
+constexpr int A_BYTES = BM * BK * 2;   // 16 KB
+constexpr int B_BYTES = BN * BK * 2;   // 32 KB
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int MN_BOX_BYTES = 64 * BK * 2;  // one 64(MN) x 64(K) box of an MN-major operand: 8 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int NTHREADS = 192;
+constexpr int TMEM_COLS = 512;
+
+// ---------------------------------------------------------------------------------------------
+// PTX wrappers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-extern "C" int32_t moe_quantize_weight(const void*, int32_t, int32_t, int32_t, int32_t, uint8_t*, float*, void*) {
-  return MOE_ERR_UNSUPPORTED;
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+      "l"(map), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem], bf16 x bf16 -> fp32
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// mbarrier arrive when all previously issued tcgen05.mma of this thread have completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns -> 32 registers per thread (thread = TMEM lane = tile row)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+        "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+        "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor (64-bit): start address, leading / stride byte offsets (all >> 4),
+// version = 1 (sm_100), layout type 2 = 128-byte swizzle.
+//   K-major tile  (rows x 64 elements, 128 B per row): 8-row groups are 1024 B apart (SBO); LBO unused.
+//   MN-major tile (64(MN) x 64(K) boxes, 128 B per k row): 8-k groups 1024 B apart (SBO); the next
+//   64 MN elements are one box (8192 B) further (LBO).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;   // descriptor version (Blackwell)
+  d |= (uint64_t)2 << 61;   // SWIZZLE_128B
+  return d;
+}
+// Instruction descriptor for kind::f16: D fp32, A/B bf16, M = 128, N = BN; majors: 0 = K-major, 1 = MN-major.
+__host__ __device__ constexpr uint32_t instr_desc(int a_mn, int b_mn) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) |
+         ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
+// ---------------------------------------------------------------------------------------------
+// kernel parameters
+// ---------------------------------------------------------------------------------------------
+struct TcParams {
+  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0;
+  int64_t rows_valid;
+  const int32_t* mtile;
+  const int32_t* offsets;
+  __nv_bfloat16* out0;
+  int64_t ld0;
+  __nv_bfloat16* out1;
+  int64_t ld1;
+  const __nv_bfloat16* gu;
+  int64_t ldgu;
+};
+
+struct Tile {
+  int e, m0, n0, nkb, row0;
+};
+
+template <int MODE>
+__device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_t total, Tile& tl) {
+  if (t >= total) return false;
+  if (MODE == TC_WGRAD) {
+    const int per_e = p.m_tiles * p.n_tiles;
+    tl.e = (int)(t / per_e);
+    const int r = (int)(t - (int64_t)tl.e * per_e);
+    tl.m0 = (r / p.n_tiles) * BM;
+    tl.n0 = (r % p.n_tiles) * BN;
+    if (p.mtile) {
+      tl.row0 = p.offsets[tl.e];
+      tl.nkb = (p.offsets[tl.e + 1] - tl.row0) / BK;
+    } else {
+      tl.row0 = 0;
+      tl.nkb = (int)((p.rows_valid + BK - 1) / BK);
+    }
+  } else {
+    const int mt = (int)(t / p.n_tiles);
+    tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
+    tl.m0 = mt * BM;
+    tl.e = p.mtile ? p.mtile[1 + mt] : 0;
+    tl.nkb = p.nkb;
+    tl.row0 = 0;
+  }
+  return true;
+}
+
+template <int MODE>
+__device__ __forceinline__ int64_t total_tiles(const TcParams& p) {
+  if (MODE == TC_WGRAD) return (int64_t)p.E * p.m_tiles * p.n_tiles;
+  const int64_t mt = p.mtile ? p.mtile[0] : (p.rows_valid + BM - 1) / BM;
+  return mt * p.n_tiles;
+}
+
+// ---------------------------------------------------------------------------------------------
+// epilogues: thread = tile row (TMEM lane); 32-column chunks; direct 16-byte global stores
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void store_row_chunk(__nv_bfloat16* dst, const uint32_t (&v)[32], int ncols) {
+  // dst: first of 32 output columns of this thread's row (16-byte aligned); ncols valid (multiple of 8)
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (q * 8 < ncols) {
+      uint4 o;
+      o.x = pack_bf16(__uint_as_float(v[q * 8 + 0]), __uint_as_float(v[q * 8 + 1]));
+      o.y = pack_bf16(__uint_as_float(v[q * 8 + 2]), __uint_as_float(v[q * 8 + 3]));
+      o.z = pack_bf16(__uint_as_float(v[q * 8 + 4]), __uint_as_float(v[q * 8 + 5]));
+      o.w = pack_bf16(__uint_as_float(v[q * 8 + 6]), __uint_as_float(v[q * 8 + 7]));
+      *reinterpret_cast<uint4*>(dst + q * 8) = o;
+    }
+  }
+}
+
+__device__ __forceinline__ float fast_sigmoid(float x) { return 1.0f / (1.0f + __expf(-x)); }
+
+template <int MODE>
+__device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
+                                              bool have_acc) {
+  // tacc: TMEM address of this warp's lane group at the accumulator stage's first column
+  if (MODE == TC_FWD || MODE == TC_DGRAD) {
+    const int64_t row = (int64_t)tl.m0 + row_in_tile;
+    const bool row_ok = row < p.rows_valid;
+    __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0;
+#pragma unroll 1
+    for (int c = 0; c < BN / 32; ++c) {
+      const int ncols = p.N - (tl.n0 + c * 32);   // warp-uniform
+      if (ncols <= 0) break;
+      uint32_t v[32];
+      tmem_ld32(tacc + c * 32, v);
+      tmem_ld_wait();
+      if (row_ok) store_row_chunk(dst + c * 32, v, ncols);
+    }
+  } else if (MODE == TC_WGRAD) {
+    const int m = tl.m0 + row_in_tile;
+    const bool row_ok = m < p.M;
+    __nv_bfloat16* dst = p.out0 + ((int64_t)tl.e * p.M + m) * p.ld0 + tl.n0;
+#pragma unroll 1
+    for (int c = 0; c < BN / 32; ++c) {
+      const int ncols = p.N - (tl.n0 + c * 32);
+      if (ncols <= 0) break;
+      uint32_t v[32];
+      if (have_acc) {
+        tmem_ld32(tacc + c * 32, v);
+        tmem_ld_wait();
+      } else {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) v[i] = 0u;   // empty expert: exact zeros
+      }
+      if (row_ok) store_row_chunk(dst + c * 32, v, ncols);
+    }
+  } else if (MODE == TC_FWD_SWIGLU) {
+    // accumulator columns [0,128) = gate, [128,256) = up for output columns n0 .. n0+127
+    const int64_t row = (int64_t)tl.m0 + row_in_tile;
+    const bool row_ok = row < p.rows_valid;
+    __nv_bfloat16* gdst = p.out0 + row * p.ld0 + tl.n0;
+    __nv_bfloat16* udst = gdst + p.F;
+    __nv_bfloat16* adst = p.out1 + row * p.ld1 + tl.n0;
+#pragma unroll 1
+    for (int c = 0; c < BN / 64; ++c) {
+      const int ncols = p.F - (tl.n0 + c * 32);
+      if (ncols <= 0) break;
+      uint32_t g[32], u[32];
+      tmem_ld32(tacc + c * 32, g);
+      tmem_ld32(tacc + BN / 2 + c * 32, u);
+      tmem_ld_wait();
+      if (row_ok) {
+        store_row_chunk(gdst + c * 32, g, ncols);
+        store_row_chunk(udst + c * 32, u, ncols);
+      }
+#pragma unroll
+      for (int i = 0; i < 32; ++i) {
+        const float gv = __uint_as_float(g[i]);
+        g[i] = __float_as_uint(gv * fast_sigmoid(gv) * __uint_as_float(u[i]));
+      }
+      if (row_ok) store_row_chunk(adst + c * 32, g, ncols);
+    }
+  } else {  // TC_DGRAD_SWIGLU: acc = da [128 x 256 columns of F]
+    const int64_t row = (int64_t)tl.m0 + row_in_tile;
+    const bool row_ok = row < p.rows_valid;
+    const __nv_bfloat16* gsrc = p.gu + row * p.ldgu + tl.n0;
+    __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + tl.n0;
+#pragma unroll 1
+    for (int c = 0; c < BN / 32; ++c) {
+      const int ncols = p.F - (tl.n0 + c * 32);
+      if (ncols <= 0) break;
+      uint32_t d[32];
+      tmem_ld32(tacc + c * 32, d);
+      tmem_ld_wait();
+      if (row_ok) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (q * 8 < ncols) {
+            const uint4 gq = *reinterpret_cast<const uint4*>(gsrc + c * 32 + q * 8);
+            const uint4 uq = *reinterpret_cast<const uint4*>(gsrc + p.F + c * 32 + q * 8);
+            const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
+            uint32_t og[4], ou[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+              const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
+              const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
+              og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
+              ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
+            }
+            *reinterpret_cast<uint4*>(dgdst + c * 32 + q * 8) = make_uint4(og[0], og[1], og[2], og[3]);
+            *reinterpret_cast<uint4*>(dgdst + p.F + c * 32 + q * 8) = make_uint4(ou[0], ou[1], ou[2], ou[3]);
+          }
+        }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
+               const __grid_constant__ CUtensorMap tmB1, const TcParams p) {
+  constexpr bool A_MN = (MODE == TC_WGRAD);
+  constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128-byte swizzle wants 1024-byte alignment
+  const uint32_t bars = base + STAGES * STAGE_BYTES;
+  // barrier addresses: full[s] = bars + 8 s; empty[s] = bars + 8 (STAGES + s); tfull[a] / tempty[a] follow
+  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
+  const uint32_t tmem_slot = tempty0 + 16;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB0);
+    tma_prefetch_desc(&tmB1);
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(tfull0 + 8 * a, 1);
+      mbar_init(tempty0 + 8 * a, 4);   // one arrive per epilogue warp
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int64_t total = total_tiles<MODE>(p);
+
+  if (warp == 0) {
+    // ===================== TMA producer (one thread) =====================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      Tile tl;
+      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+        for (int kb = 0; kb < tl.nkb; ++kb) {
+          mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const uint32_t fb = full0 + 8 * stage;
+          const uint32_t sa = base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          mbar_expect_tx(fb, STAGE_BYTES);
+          if (!A_MN) {
+            tma_load_2d(sa, &tmA, fb, kb * BK, tl.m0);                              // box 64 x 128
+          } else {
+            const int kr = tl.row0 + kb * BK;
+#pragma unroll
+            for (int i = 0; i < BM / 64; ++i) tma_load_2d(sa + i * MN_BOX_BYTES, &tmA, fb, p.a_col0 + tl.m0 + 64 * i, kr);
+          }
+          if (MODE == TC_FWD) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 256
+          } else if (MODE == TC_FWD_SWIGLU) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 128 (Wg)
+            tma_load_2d(sb + B_BYTES / 2, &tmB1, fb, kb * BK, tl.e * p.b_rows + tl.n0);  // (Wu)
+          } else if (MODE == TC_WGRAD) {
+            const int kr = tl.row0 + kb * BK;
+#pragma unroll
+            for (int i = 0; i < BN / 64; ++i) tma_load_2d(sb + i * MN_BOX_BYTES, &tmB0, fb, tl.n0 + 64 * i, kr);
+          } else {
+            const bool second = kb >= p.kb_split;
+            const CUtensorMap* bm = second ? &tmB1 : &tmB0;
+            const int kr = tl.e * p.b_rows + (second ? kb - p.kb_split : kb) * BK;
+#pragma unroll
+            for (int i = 0; i < BN / 64; ++i) tma_load_2d(sb + i * MN_BOX_BYTES, bm, fb, tl.n0 + 64 * i, kr);
+          }
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one thread) =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = instr_desc(A_MN ? 1 : 0, B_MN ? 1 : 0);
+      int stage = 0, as = 0;
+      uint32_t phase = 0, aphase = 0;
+      Tile tl;
+      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+        if (tl.nkb == 0) continue;
+        mbar_wait(tempty0 + 8 * as, aphase ^ 1);
+        tc_fence_after();
+        const uint32_t dacc = tmem_base + as * BN;
+        for (int kb = 0; kb < tl.nkb; ++kb) {
+          mbar_wait(full0 + 8 * stage, phase);
+          tc_fence_after();
+          const uint32_t sa = base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < BK / UK; ++k) {
+            const uint64_t ad = A_MN ? smem_desc(sa + k * UK * 128, MN_BOX_BYTES, 1024) : smem_desc(sa + k * UK * 2, 16, 1024);
+            const uint64_t bd = B_MN ? smem_desc(sb + k * UK * 128, MN_BOX_BYTES, 1024) : smem_desc(sb + k * UK * 2, 16, 1024);
+            umma_bf16(dacc, ad, bd, idesc, (kb | k) != 0);
+          }
+          umma_commit(empty0 + 8 * stage);   // frees the smem stage once these MMAs have read it
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        umma_commit(tfull0 + 8 * as);        // accumulator complete
+        if (++as == 2) { as = 0; aphase ^= 1; }
+      }
+    }
+  } else {
+    // ===================== epilogue warps 2..5 =====================
+    const int lg = warp & 3;                 // TMEM lane group this warp may access
+    const int row_in_tile = lg * 32 + lane;
+    int as = 0;
+    uint32_t aphase = 0;
+    Tile tl;
+    for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      const bool have = tl.nkb > 0;
+      if (have) {
+        mbar_wait(tfull0 + 8 * as, aphase);
+        tc_fence_after();
+      }
+      const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + as * BN;
+      epilogue_tile<MODE>(p, tl, tacc, row_in_tile, have);
+      if (have) {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+        if (++as == 2) { as = 0; aphase ^= 1; }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host: tensor maps and launch
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(sym);
+    else
+      cudaGetLastError();
+  }
+  return fn;
+}
+
+// 2-D bf16 tensor [outer, inner] (inner contiguous, row pitch ld elements), box = box_outer x 64, 128-byte swizzle,
+// out-of-bounds elements read as zero.
+bool make_map(CUtensorMap* m, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_outer) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn || !ptr || inner <= 0 || outer <= 0) return false;
+  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || ((ld * 2) & 15)) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_outer};
+  const cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int g_sm_count = 0;
+bool g_attr_set[5] = {false, false, false, false, false};
+
+template <int MODE>
+int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const TcParams& p, int64_t max_tiles,
+               cudaStream_t s) {
+  if (!g_attr_set[MODE]) {
+    MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    g_attr_set[MODE] = true;
+  }
+  if (g_sm_count == 0) {
+    int dev = 0;
+    MOE_CUDA(cudaGetDevice(&dev));
+    MOE_CUDA(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
+  }
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(g_sm_count, max_tiles));
+  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, p);
+  return MOE_OK;
+}
+
+// mtile[0] = number of 128-row tiles below offsets[E]; mtile[1 + i] = expert owning tile i.
+__global__ void prepare_tiles_kernel(const int32_t* __restrict__ offsets, int E, int32_t* __restrict__ mtile) {
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    const int lo = offsets[e] / BM, hi = offsets[e + 1] / BM;
+    for (int t = lo; t < hi; ++t) mtile[1 + t] = e;
+  }
+  if (threadIdx.x == 0) mtile[0] = offsets[E] / BM;
+}
+
+}  // namespace
+
+int32_t tc_prepare_tiles(const int32_t* offsets, int E, int64_t rows_cap, int32_t* mtile_expert, cudaStream_t s) {
+  (void)rows_cap;
+  MOE_LAUNCH(prepare_tiles_kernel, 1, 256, 0, s, offsets, E, mtile_expert);
+  return MOE_OK;
+}
+
+int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
+  if (c.mtile == nullptr && c.E != 1) return MOE_ERR_UNSUPPORTED;
+  TcParams p;
+  memset(&p, 0, sizeof(p));
+  p.E = c.E;
+  p.rows_valid = c.rows_cap;
+  p.mtile = c.mtile;
+  p.offsets = c.offsets;
+  p.out0 = (__nv_bfloat16*)c.out0;
+  p.ld0 = c.ld0;
+  p.out1 = (__nv_bfloat16*)c.out1;
+  p.ld1 = c.ld1;
+  p.gu = (const __nv_bfloat16*)c.gu;
+  p.ldgu = c.ldgu;
+  p.F = c.F;
+  p.N = c.N;
+  p.M = c.M;
+  p.b_rows = c.b_rows;
+  p.a_col0 = c.a_col0;
+  CUtensorMap ta, tb0, tb1;
+  const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
+  if ((c.N & 7) || (c.ld0 & 7)) return MOE_ERR_UNSUPPORTED;
+  switch (c.mode) {
+    case TC_FWD: {
+      if (c.Kd % BK) return MOE_ERR_UNSUPPORTED;
+      p.nkb = c.Kd / BK;
+      p.n_tiles = (int)ceil_div(c.N, BN);
+      if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
+      return launch<TC_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
+    }
+    case TC_FWD_SWIGLU: {
+      if (c.Kd % BK || (c.F & 7) || (c.ld1 & 7)) return MOE_ERR_UNSUPPORTED;
+      p.nkb = c.Kd / BK;
+      p.n_tiles = (int)ceil_div(c.F, BN / 2);
+      if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb1, c.B1, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
+      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+    }
+    case TC_DGRAD:
+    case TC_DGRAD_SWIGLU: {
+      // contraction over the weights' rows (b_rows per source), output columns = b_cols
+      if (c.b_rows % BK) return MOE_ERR_UNSUPPORTED;
+      const bool split = c.B1 != nullptr;
+      p.kb_split = c.b_rows / BK;
+      p.nkb = split ? 2 * p.kb_split : p.kb_split;
+      p.n_tiles = (int)ceil_div(c.N, BN);
+      if (!make_map(&ta, c.A, (int64_t)p.nkb * BK, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb1, split ? c.B1 : c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
+      if (c.mode == TC_DGRAD) return launch<TC_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      if ((c.F & 7) || (c.ldgu & 7)) return MOE_ERR_UNSUPPORTED;
+      return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+    }
+    case TC_WGRAD: {
+      p.m_tiles = (int)ceil_div(c.M, BM);
+      p.n_tiles = (int)ceil_div(c.N, BN);
+      // A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (inner = output columns)
+      if (!make_map(&ta, c.A, c.lda, c.rows_cap, c.lda, 64)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&tb0, c.A2, c.N, c.rows_cap, c.lda2, 64)) return MOE_ERR_UNSUPPORTED;
+      return launch<TC_WGRAD>(ta, tb0, tb0, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
+    }
+  }
+  return MOE_ERR_INVALID_ARG;
+}
+
+}  // namespace moe

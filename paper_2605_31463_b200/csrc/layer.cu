@@ -1,7 +1,9 @@
 // moe_layer_fwd / moe_layer_bwd: composition of the hot path (SURVEY.md §3 call stack, §8c R1..R8),
 // plus the public grouped-GEMM entry points.  Single stream, no host synchronisation anywhere:
 // per-expert counts stay on the device.
-#include "common.cuh"
+#include <string.h>
+
+#include "gemm_tc.cuh"
 
 namespace moe {
 
@@ -14,13 +16,8 @@ struct FfnGroup {
   const int32_t* counts;   // [E] device or nullptr (then offsets differences are used)
   const int32_t* mtile;    // M-tile -> expert table (tensor-core path) or nullptr
   int row_align;
+  int st_fwd1, st_fwd2, st_bwd1, st_bwd2, st_wgrad;  // profile stages of the five GEMM groups
 };
-
-int32_t tc_ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* Wu, const void* Wd, void* gu,
-                   void* a, void* y, cudaStream_t s);
-int32_t tc_ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* gu, const void* a, const void* Wg,
-                   const void* Wu, const void* Wd, void* dgu, void* dXp, void* dWg, void* dWu, void* dWd,
-                   cudaStream_t s);
 
 namespace {
 
@@ -29,18 +26,45 @@ __global__ void set2_kernel(int32_t* p, int32_t a, int32_t b) {
   p[1] = b;
 }
 
+// tcgen05 path: bf16, H and F multiples of 64, and either 128-row-aligned groups or a single group.
+bool use_tc(const FfnGroup& g) {
+  return g.dtype == 1 && g.H % 64 == 0 && g.F % 64 == 0 && (g.mtile != nullptr || g.E == 1);
+}
+
+TcCall tc_base(const FfnGroup& g, int mode) {
+  TcCall c;
+  memset(&c, 0, sizeof(c));
+  c.mode = mode;
+  c.E = g.E;
+  c.rows_cap = g.rows_cap;
+  c.offsets = g.offsets;
+  c.mtile = g.mtile;
+  c.F = g.F;
+  return c;
+}
+
 int32_t ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* Wu, const void* Wd, void* gu, void* a,
                 void* y, cudaStream_t s) {
-  if (g.dtype != 0) {
-    const int32_t st = tc_ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s);
-    if (st != MOE_ERR_UNSUPPORTED) return st;
+  if (use_tc(g)) {
+    TcCall c = tc_base(g, TC_FWD_SWIGLU);   // gu = [Xp Wg^T | Xp Wu^T], a = silu(g) * u
+    c.A = Xp; c.lda = g.H; c.B0 = Wg; c.B1 = Wu; c.b_rows = g.F; c.b_cols = g.H; c.N = g.F; c.Kd = g.H;
+    c.out0 = gu; c.ld0 = 2 * g.F; c.out1 = a; c.ld1 = g.F;
+    MOE_CHECK(tc_gemm(c, s));
+    prof_mark(g.st_fwd1, s);
+    c = tc_base(g, TC_FWD);                 // y = a Wd^T
+    c.A = a; c.lda = g.F; c.B0 = Wd; c.b_rows = g.H; c.b_cols = g.F; c.N = g.H; c.Kd = g.F; c.out0 = y; c.ld0 = g.H;
+    MOE_CHECK(tc_gemm(c, s));
+    prof_mark(g.st_fwd2, s);
+    return MOE_OK;
   }
   const size_t es = g.dtype == 0 ? 4 : 2;
   MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.F, g.H, Xp, g.H, Wg, nullptr, 0, g.offsets, gu, 2 * g.F, g.rows_cap, 0, s));
   MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.F, g.H, Xp, g.H, Wu, nullptr, 0, g.offsets, (char*)gu + g.F * es,
                               2 * g.F, g.rows_cap, 0, s));
   MOE_CHECK(swiglu_fwd(g.dtype, gu, a, g.rows_cap, g.F, s));
+  prof_mark(g.st_fwd1, s);
   MOE_CHECK(simt_grouped_gemm(0, g.dtype, g.E, g.H, g.F, a, g.F, Wd, nullptr, 0, g.offsets, y, g.H, g.rows_cap, 0, s));
+  prof_mark(g.st_fwd2, s);
   return MOE_OK;
 }
 
@@ -48,22 +72,44 @@ int32_t ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* W
 int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* gu, const void* a, const void* Wg,
                 const void* Wu, const void* Wd, void* da_tmp, void* dgu, void* dXp, void* dWg, void* dWu, void* dWd,
                 cudaStream_t s) {
-  if (g.dtype != 0) {
-    const int32_t st = tc_ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, dgu, dXp, dWg, dWu, dWd, s);
-    if (st != MOE_ERR_UNSUPPORTED) return st;
-  }
   const size_t es = g.dtype == 0 ? 4 : 2;
   const void* dgu_u = (const char*)dgu + g.F * es;
+  if (use_tc(g)) {
+    TcCall c = tc_base(g, TC_DGRAD_SWIGLU);   // dgu = swiglu'(gu) * (dy Wd[e])
+    c.A = dy; c.lda = g.H; c.B0 = Wd; c.b_rows = g.H; c.b_cols = g.F; c.N = g.F; c.gu = gu; c.ldgu = 2 * g.F;
+    c.out0 = dgu; c.ld0 = 2 * g.F;
+    MOE_CHECK(tc_gemm(c, s));
+    prof_mark(g.st_bwd1, s);
+    c = tc_base(g, TC_DGRAD);                 // dXp = dg Wg[e] + du Wu[e]: one contraction over [dg|du]
+    c.A = dgu; c.lda = 2 * g.F; c.B0 = Wg; c.B1 = Wu; c.b_rows = g.F; c.b_cols = g.H; c.N = g.H; c.out0 = dXp; c.ld0 = g.H;
+    MOE_CHECK(tc_gemm(c, s));
+    prof_mark(g.st_bwd2, s);
+    if (dWd) {
+      c = tc_base(g, TC_WGRAD);               // dWd[e] = dy_e^T a_e
+      c.A = dy; c.lda = g.H; c.M = g.H; c.A2 = a; c.lda2 = g.F; c.N = g.F; c.out0 = dWd; c.ld0 = g.F;
+      MOE_CHECK(tc_gemm(c, s));
+      c = tc_base(g, TC_WGRAD);               // dWg[e] = dg_e^T Xp_e, dWu[e] = du_e^T Xp_e
+      c.A = dgu; c.lda = 2 * g.F; c.M = g.F; c.A2 = Xp; c.lda2 = g.H; c.N = g.H; c.out0 = dWg; c.ld0 = g.H;
+      MOE_CHECK(tc_gemm(c, s));
+      c.a_col0 = g.F; c.out0 = dWu;
+      MOE_CHECK(tc_gemm(c, s));
+      prof_mark(g.st_wgrad, s);
+    }
+    return MOE_OK;
+  }
   // da = dy Wd[e]            (B = Wd [E,H,F]: N = H, Kdim = F)
   MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.H, g.F, nullptr, 0, Wd, dy, g.H, g.offsets, da_tmp, g.F, g.rows_cap, 0, s));
   MOE_CHECK(swiglu_bwd(g.dtype, gu, da_tmp, dgu, g.rows_cap, g.F, s));
+  prof_mark(g.st_bwd1, s);
   // dXp = dg Wg[e] + du Wu[e]  (B = Wg [E,F,H]: N = F, Kdim = H)
   MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wg, dgu, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 0, s));
   MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wu, dgu_u, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 1, s));
+  prof_mark(g.st_bwd2, s);
   if (dWd) {
     MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.H, g.F, a, g.F, nullptr, dy, g.H, g.offsets, dWd, 0, g.rows_cap, 0, s));
     MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu, 2 * g.F, g.offsets, dWg, 0, g.rows_cap, 0, s));
     MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu_u, 2 * g.F, g.offsets, dWu, 0, g.rows_cap, 0, s));
+    prof_mark(g.st_wgrad, s);
   }
   return MOE_OK;
 }
@@ -102,24 +148,32 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
   void* a = at<char>(ctx, C.a);
   void* y = at<char>(ctx, C.y);
 
+  prof_mark(ST_BEGIN, s);
   MOE_CHECK(router_logits(cfg, X, Wr, z, s));                                              // R1
+  prof_mark(ST_ROUTER_GEMM, s);
   MOE_CHECK(moe_route(cfg, z, bias, topk_idx, topk_w, stream));                            // R2..R5
   MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.idx), topk_idx, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
   MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.w), topk_w, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
+  prof_mark(ST_ROUTE, s);
   MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, p2f, f2p, mtile, at<int32_t>(ws, W.hist), s));  // R6
+  prof_mark(ST_MAPS, s);
   MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, Xp, s));
+  prof_mark(ST_PERMUTE, s);
   FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
-             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align};
+             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
+             ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
   MOE_CHECK(ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s));                                      // R7
   const void* shared_out = nullptr;
   if (shared) {
     int32_t* off_s = offsets + cfg->E + 1;
     MOE_LAUNCH(set2_kernel, 1, 1, 0, s, off_s, 0, cfg->T);
-    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1};
+    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
+                ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
     MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
     shared_out = at<char>(ctx, C.y_s);
   }
   MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, Y, s));    // R7 combine
+  prof_mark(ST_COMBINE, s);
   return MOE_OK;
 }
 
@@ -159,20 +213,26 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   void* dXp = at<char>(ws, W.dXp);
   void* tmp = at<char>(ws, W.tmp);
 
+  prof_mark(ST_BEGIN, s);
   MOE_CHECK(combine_bwd(cfg, dY, y, w, f2p, p2f, offsets, dy, dw, s));                     // R8 combine-bwd
+  prof_mark(ST_COMBINE_BWD, s);
   FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
-             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align};
+             (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
+             ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
   MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));       // R8 expert FFN
   MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, Xp, dz, dzp, dWr, s));    // R8 router
+  prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
   if (shared) {
     const int32_t* off_s = offsets + cfg->E + 1;
-    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1};
+    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
+                ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
     MOE_CHECK(ffn_bwd(gs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), Wg_s, Wu_s, Wd_s, tmp,
                       at<char>(ws, W.dgu_s), at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
     dXs = at<char>(ws, W.dXs);
   }
   // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]
   MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, dz, idx, Wr, dX, s));
+  prof_mark(ST_DX_COMBINE, s);
   return MOE_OK;
 }

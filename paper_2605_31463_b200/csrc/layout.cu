@@ -179,3 +179,53 @@ extern "C" int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_
     }
   return MOE_ERR_INVALID_ARG;
 }
+
+// ---- stage timing -------------------------------------------------------------------------------------
+namespace moe {
+int g_prof_on = 0;
+namespace {
+constexpr int MAX_MARKS = 8192;
+cudaEvent_t g_ev[MAX_MARKS];
+int g_ev_stage[MAX_MARKS];
+int g_ev_created = 0, g_ev_used = 0;
+const char* const kStageNames[ST_COUNT] = {"begin", "router_gemm", "route", "maps", "permute", "gemm1_swiglu", "gemm2",
+                                           "combine", "combine_bwd", "dgrad_down_swiglu", "dgrad_gateup", "wgrad",
+                                           "router_bwd", "dx_combine", "shared_fwd", "shared_bwd", "quant"};
+}  // namespace
+void prof_mark_impl(int stage, cudaStream_t s) {
+  if (g_ev_used >= MAX_MARKS) return;
+  if (g_ev_used >= g_ev_created) {
+    if (cudaEventCreate(&g_ev[g_ev_created]) != cudaSuccess) { cudaGetLastError(); return; }
+    ++g_ev_created;
+  }
+  g_ev_stage[g_ev_used] = stage;
+  cudaEventRecord(g_ev[g_ev_used++], s);
+}
+}  // namespace moe
+
+extern "C" int32_t moe_profile_enable(int32_t on) {
+  g_prof_on = on ? 1 : 0;
+  g_ev_used = 0;
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_profile_stage_ms(const char* stage, double* total_ms, int64_t* segments) {
+  if (!stage || !total_ms || !segments) return MOE_ERR_INVALID_ARG;
+  int want = -1;
+  for (int i = 1; i < ST_COUNT; ++i)
+    if (strcmp(kStageNames[i], stage) == 0) want = i;
+  if (want < 0) return MOE_ERR_INVALID_ARG;
+  double sum = 0;
+  int64_t n = 0;
+  for (int i = 1; i < g_ev_used; ++i) {
+    if (g_ev_stage[i] != want) continue;
+    if (cudaEventSynchronize(g_ev[i]) != cudaSuccess) { cudaGetLastError(); return MOE_ERR_CUDA; }
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g_ev[i - 1], g_ev[i]) != cudaSuccess) { cudaGetLastError(); return MOE_ERR_CUDA; }
+    sum += ms;
+    ++n;
+  }
+  *total_ms = sum;
+  *segments = n;
+  return MOE_OK;
+}

@@ -1,0 +1,69 @@
+"""CPU checks of the boundary: the C-ABI library loads and exports every symbol include/moe_b200.h declares,
+and the host-only entry points (status strings, size queries, argument validation) behave as documented.
+No compute call is made (no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "moe_b200.h")
+
+
+@pytest.fixture(scope="module")
+def moe():
+    import __graft_entry__ as ge
+    ge.build()
+    import paper_2605_31463_b200 as m
+    return m
+
+
+def declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(moe_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_declares_north_star_calls():
+    names = declared_symbols()
+    for need in ("moe_route", "moe_permute", "moe_grouped_gemm_fwd", "moe_grouped_gemm_bwd", "moe_swiglu",
+                 "moe_unpermute_combine", "moe_layer_fwd", "moe_layer_bwd"):
+        assert need in names
+
+
+def test_library_exports_every_declared_symbol(moe):
+    lib = C.CDLL(moe.LIB_PATH)
+    for name in declared_symbols():
+        assert hasattr(lib, name), f"{name} declared in moe_b200.h but not exported"
+    assert set(declared_symbols()) == set(moe.EXPORTS)
+
+
+def test_status_strings_and_version(moe):
+    assert moe.moe_version() >= 100
+    seen = {moe.status_string(s) for s in (0, -1, -2, -3, -4)}
+    assert len(seen) == 5
+
+
+@pytest.mark.parametrize("cfg", list(wl.CONFIGS.values()) + list(wl.SMALL_CONFIGS.values()), ids=lambda c: c.name)
+def test_size_queries(moe, cfg):
+    for align in (1, 128):
+        c = cfg.replace(row_align=align)
+        assert moe.moe_padded_rows(c) == c.TK_pad
+        ws, ctx = moe.moe_workspace_bytes(c)
+        assert ws > 0 and ctx > 0 and ws % 256 == 0 and ctx % 256 == 0
+        off, ln = moe.moe_ctx_field(c, "flat_to_perm")
+        assert ln == c.TK * 4 and off + ln <= ctx
+
+
+def test_invalid_configs_are_rejected_on_the_host(moe):
+    bad = [wl.TINY.replace(K=9), wl.TINY.replace(T=0), wl.TINY.replace(n_group=3),
+           wl.DSV3_SMALL.replace(topk_group=1, K=16), wl.TINY.replace(score_fn=7)]
+    for c in bad:
+        with pytest.raises(moe.MoEError):
+            moe.moe_workspace_bytes(c)
+    # NULL pointers: INVALID_ARG before anything is enqueued (no CUDA call happens)
+    st = moe.lib().moe_route(C.byref(moe.make_config(wl.TINY)), None, None, None, None, None)
+    assert st == moe.MOE_ERR_INVALID_ARG
