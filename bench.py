@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- MoE layer fwd+bwd throughput on B200 through the C ABI (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
+
+One "step" = moe_layer_fwd + moe_layer_bwd (every row of SURVEY.md §8a) over one batch of synthetic input.
+Prints ONE JSON line (rank 0).  `value` = algorithmic TFLOP/s (18*T*K*H*F + shared + router flops, S20)
+with inputs resident in HBM; `e2e` = the same through moe_layer_step_host with pinned HOST activations
+(H2D of X, dY and D2H of Y, dX inside the timed region).  Multi-GPU: replicas only: each rank
+runs the same layer on its own batch, no data-path collective, weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+METRIC = "moe_layer_fwd_bwd_tflops"
+UNIT = "TFLOP/s"
+NOMINAL = {"bf16_tflops": 2250.0, "hbm_gbs": 8000.0}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_burst": p["bf16_tflops"], "bf16_sustained": p["bf16_tflops_sustained"],
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def pick_config(name):
+    cfg = wl.CONFIGS.get(name) or wl.SMALL_CONFIGS.get(name)
+    if cfg is None:
+        raise SystemExit(f"unknown config {name}; have {sorted(wl.CONFIGS) + sorted(wl.SMALL_CONFIGS)}")
+    if cfg.dtype != wl.DTYPE_FP32:
+        cfg = cfg.replace(row_align=128)   # tensor-core path: expert groups start at multiples of 128 rows
+    return cfg
+
+
+# ----------------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline and --impl reference): a bounded sample of the same workload
+# ----------------------------------------------------------------------------------------------------
+
+def oracle_sample(cfg, budget_s=12.0, max_experts=24):
+    """Oracle routing over all T tokens, then the oracle's expert FFN fwd+bwd (fp64) for experts 0..n-1 on the
+    rows routed to them, until `budget_s` of CPU time is spent.  Returns (flops, seconds, description)."""
+    from oracle import moe_oracle as orc
+    X, Wr, bias, dY = wl.gen_X(cfg), wl.gen_Wr(cfg), wl.gen_bias(cfg), wl.gen_dY(cfg)
+    t0 = time.perf_counter()
+    z = orc.router_logits(X, Wr)
+    idx, w = orc.route(z, bias, cfg)
+    counts, offsets, p2f, f2p = orc.permute_maps(idx, cfg.E, 1)
+    Xp = orc.permute_rows(X, p2f, cfg.K)
+    t_route = time.perf_counter() - t0
+    flops = 2.0 * cfg.T * cfg.H * cfg.E
+    spent, n, rows = t_route, 0, 0
+    for e in range(min(cfg.E, max_experts)):
+        Wg, Wu, Wd = wl.gen_expert_weights(cfg, e)            # generation is not timed
+        r0, r1 = int(offsets[e]), int(offsets[e]) + int(counts[e])
+        if r1 == r0:
+            continue
+        t0 = time.perf_counter()
+        g, u, a, y = orc.expert_ffn_fwd(Xp[r0:r1], Wg, Wu, Wd)
+        tok = p2f[r0:r1] // cfg.K
+        dy = dY[tok].astype(np.float64) * w.reshape(-1)[p2f[r0:r1]][:, None]
+        orc.expert_ffn_bwd(dy, Xp[r0:r1], g, u, a, Wg, Wu, Wd)
+        spent += time.perf_counter() - t0
+        flops += 18.0 * (r1 - r0) * cfg.H * cfg.F
+        n += 1
+        rows += r1 - r0
+        if spent > budget_s:
+            break
+    return flops, spent, f"oracle routing of all {cfg.T} tokens + expert FFN fwd+bwd (fp64) of experts 0..{n - 1} ({rows} routed rows)"
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([i.get("num_threads", 1) for i in threadpool_info()] or [os.cpu_count()])
+    except Exception:
+        return os.cpu_count()
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle_sample(cfg, budget_s=1.0, max_experts=1)
+    budget = max(2.0, min(12.0, 120.0 / max(1, args.steps)))
+    tot_f = tot_t = 0.0
+    desc = ""
+    for _ in range(args.steps):
+        f, t, desc = oracle_sample(cfg, budget_s=budget)
+        tot_f += f
+        tot_t += t
+    val = tot_f / tot_t / 1e12
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": tot_t / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "T": cfg.T, "H": cfg.H, "E": cfg.E, "K": cfg.K, "F": cfg.F},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ----------------------------------------------------------------------------------------------------
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.01):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.stop_flag = period, [], set(), False
+        self.max_mhz, self.power = None, []
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv, self.h = nv, nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake_slowdown": 0x80}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s), "power_w_max": (max(self.power) if self.power else None)}
+
+
+def stage_flops(cfg):
+    """Algorithmic flops per stage per step (S20)."""
+    r = cfg.T * cfg.K * cfg.H * cfg.F
+    s = cfg.T * cfg.H * cfg.F_shared
+    return {"gemm1_swiglu": 4 * r, "gemm2": 2 * r, "dgrad_down_swiglu": 2 * r, "dgrad_gateup": 4 * r, "wgrad": 6 * r,
+            "shared_fwd": 6 * s, "shared_bwd": 12 * s, "router_gemm": 2 * cfg.T * cfg.H * cfg.E}
+
+
+def stage_bytes(cfg):
+    """Algorithmic HBM bytes per stage per step."""
+    b = 4 if cfg.dtype == wl.DTYPE_FP32 else 2
+    T, H, E, K, TK = cfg.T, cfg.H, cfg.E, cfg.K, cfg.T * cfg.K
+    return {"route": T * E * 4 + TK * 8, "maps": 3 * TK * 4, "permute": T * H * b + TK * H * b + TK * 4,
+            "combine": TK * H * b + T * H * b + TK * 8, "combine_bwd": 2 * TK * H * b + T * H * b + TK * 12,
+            "dx_combine": TK * H * b + T * H * b + TK * 4}
+
+
+def run_cuda(args, cfg):
+    import torch
+    import torch.distributed as dist
+    import paper_2605_31463_b200 as moe
+    from paper_2605_31463_b200.buffers import LayerBuffers, act_dtype, to_device
+    moe.lib()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = load_peaks()
+    dt = act_dtype(cfg)
+    cfg_r = cfg.replace(seed=cfg.seed + rank)              # each replica gets its own batch
+    lb = LayerBuffers(cfg)
+    lb.load(X=wl.gen_X(cfg_r), dY=wl.gen_dY(cfg_r), Wr=wl.gen_Wr(cfg), bias=wl.gen_bias(cfg))
+    g = torch.Generator(device="cuda").manual_seed(1234)
+    std = cfg.w_std if cfg.w_std > 0 else None
+    for w, fan_in in ((lb.Wg, cfg.H), (lb.Wu, cfg.H), (lb.Wd, cfg.F), (lb.Wg_s, cfg.H), (lb.Wu_s, cfg.H), (lb.Wd_s, cfg.F_shared)):
+        if w is None:
+            continue
+        for e in range(w.shape[0] if w.dim() == 3 else 1):   # expert by expert: bounded fp32 temporaries
+            dst = w[e] if w.dim() == 3 else w
+            dst.copy_(torch.randn(dst.shape, generator=g, device="cuda", dtype=torch.float32) * (std or fan_in ** -0.5))
+    stream = torch.cuda.current_stream()
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step():
+        lb.forward(stream)
+        lb.backward(stream)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    sync_all()
+    sampler = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    moe.moe_profile_enable(True)
+    n0 = moe.moe_launch_count()
+    sampler.start()
+    sync_all()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    sync_all()
+    sampler.stop_flag = True
+    launches = moe.moe_launch_count() - n0
+    ms = ev0.elapsed_time(ev1)
+    stages = {}
+    for name in moe.STAGES:
+        t, n = moe.moe_profile_stage_ms(name)
+        if n:
+            stages[name] = {"ms_per_step": t / args.steps, "segments_per_step": n / args.steps}
+    moe.moe_profile_enable(False)
+    if world > 1:
+        tmax = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
+    fl = cfg.flops_fwd_bwd()
+    value = world * fl["total"] * args.steps / (ms * 1e-3) / 1e12
+
+    # ---- end to end: host activations in, host results out, copies inside the timed region ----
+    Xh = lb.X.cpu().pin_memory(); dYh = lb.dY.cpu().pin_memory()
+    Yh = torch.empty_like(Xh).pin_memory(); dXh = torch.empty_like(Xh).pin_memory()
+    for _ in range(3):
+        lb.step_host(Xh, dYh, Yh, dXh, stream)
+    sync_all()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        lb.step_host(Xh, dYh, Yh, dXh, stream)
+    e1.record(stream)
+    sync_all()
+    ms_e2e = e0.elapsed_time(e1)
+    if world > 1:
+        tmax = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms_e2e = float(tmax.item())
+    act_bytes = cfg.T * cfg.H * (4 if cfg.dtype == wl.DTYPE_FP32 else 2)
+    e2e = {"value": world * fl["total"] * args.steps / (ms_e2e * 1e-3) / 1e12, "unit": UNIT,
+           "h2d_bytes_per_step": 2 * act_bytes, "d2h_bytes_per_step": 2 * act_bytes, "ms_per_step": ms_e2e / args.steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- stage table: TFLOP/s for the GEMMs, GB/s for the HBM-bound movers ----
+    sf, sb = stage_flops(cfg), stage_bytes(cfg)
+    for name, st in stages.items():
+        sec = st["ms_per_step"] * 1e-3
+        if name in sf and sf[name] and sec > 0:
+            st["tflops"] = sf[name] / sec / 1e12
+            st["frac_measured_sustained"] = st["tflops"] / peaks["bf16_sustained"]
+            st["frac_nominal"] = st["tflops"] / NOMINAL["bf16_tflops"]
+        if name in sb and sec > 0:
+            st["gbs"] = sb[name] / sec / 1e9
+            st["frac_measured"] = st["gbs"] / peaks["hbm_gbs"]
+            st["frac_nominal"] = st["gbs"] / NOMINAL["hbm_gbs"]
+    gemm_stages = [n for n in ("gemm1_swiglu", "gemm2", "dgrad_down_swiglu", "dgrad_gateup", "wgrad") if n in stages]
+    roofline = None
+    if gemm_stages:
+        dom = max(gemm_stages, key=lambda n: stages[n]["ms_per_step"])
+        st = stages[dom]
+        nl = 3 if dom == "wgrad" else 1
+        tc = "tflops" in st and cfg.dtype != wl.DTYPE_FP32
+        roofline = {"bound": "tensor" if tc else "alu", "kernel": dom, "achieved": st.get("tflops"),
+                    "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
+                    "frac": (st["tflops"] / peaks["bf16_sustained"]) if "tflops" in st else None,
+                    "traffic": None, "launches_per_step": nl, "ms_per_launch": st["ms_per_step"] / nl,
+                    "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
+                    "frac_nominal_2250": st.get("frac_nominal")}
+    rp = [stages[n]["ms_per_step"] for n in ("route", "maps", "permute") if n in stages]
+    route_permute = None
+    if len(rp) == 3:
+        byts = sb["route"] + sb["maps"] + sb["permute"]
+        gbs = byts / (sum(rp) * 1e-3) / 1e9
+        route_permute = {"gbs": gbs, "bytes": byts, "ms": sum(rp), "frac_measured": gbs / peaks["hbm_gbs"],
+                         "frac_nominal_8000": gbs / NOMINAL["hbm_gbs"]}
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        f, t, desc = oracle_sample(cfg)
+        cpu = {"value": f / t / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": desc,
+               "seconds": t}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.dtype], "data": "synthetic",
+            "config": {"workload": cfg.name, "T": cfg.T, "H": cfg.H, "E": cfg.E, "K": cfg.K, "F": cfg.F,
+                       "F_shared": cfg.F_shared, "row_align": cfg.row_align, "parallelism": f"replicas x{world}",
+                       "l2": "not flushed: each step streams > 1 GB of weights and activations, larger than the 126 MB L2",
+                       "inputs": "X, dY, Wr, bias from workloads (Philox, seed 0); expert weights torch.randn on device"},
+            "flops_per_step": fl, "frac_of_measured_bf16_sustained": value / world / peaks["bf16_sustained"],
+            "frac_of_nominal_bf16_2250": value / world / NOMINAL["bf16_tflops"],
+            "clocks": sampler.result(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "route_permute": route_permute, "stages": stages, "cpu_baseline": cpu, "peaks": peaks}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="qwen3_30b_a3b_like")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = pick_config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_cuda(args, cfg)
+
+
+if __name__ == "__main__":
+    main()
