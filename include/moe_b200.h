@@ -93,8 +93,8 @@ int32_t moe_permute(const moe_config_t* cfg, const void* X, const int32_t* topk_
  *   C[r, n] = sum_k A[r, k] * B[e][n, k]         A [TK_pad,Kdim], B [E,N,Kdim], C [TK_pad,N]
  * fp32 accumulation; C in the element type of A.  dtype 2: A and B are e4m3 codes (uint8) with
  * a_scales [TK_pad, Kdim/128] fp32 and b_scales [E, ceil(N/128), Kdim/128] fp32, C is bf16.
- * Rows >= offsets[E] are not touched.  Requirements for dtype 1, 2: row_align % 128 == 0, Kdim % 64 == 0
- * (dtype 2: Kdim % 128 == 0), N % 8 == 0.  */
+ * Rows >= offsets[E] are not touched.  Requirements for dtype 1: row_align % 128 == 0, Kdim % 64 == 0, N % 8 == 0
+ * (other bf16 shapes run on CUDA cores); dtype 2: row_align % 128 == 0, Kdim % 128 == 0, N % 128 == 0.  */
 int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int32_t Kdim, const void* A, const void* B,
                              const int32_t* offsets, void* C, const void* a_scales, const void* b_scales,
                              void* ws, void* stream);
@@ -131,9 +131,18 @@ int32_t moe_quantize_act(const void* v, int64_t rows, int32_t cols, int32_t scal
 int32_t moe_quantize_weight(const void* w, int32_t batch, int32_t rows, int32_t cols, int32_t scale_mode,
                             uint8_t* codes, float* scales, void* stream);
 
+/* FP8 weight cache ("FP8 weight cache"; R9 Q-W): quantise the bf16 expert weights (and the shared
+ * expert's, if any) to e4m3 codes + 128x128 block scales inside `ctx`.  moe_layer_fwd does this itself when it is
+ * given weights; call this once per optimiser step and pass Wg = Wu = Wd = NULL (and NULL shared weights) to
+ * moe_layer_fwd for the following micro-batches to reuse the codes.  cfg->dtype must be 2. */
+int32_t moe_fp8_quantize_weights(const moe_config_t* cfg, const void* Wg, const void* Wu, const void* Wd,
+                                 const void* Wg_s, const void* Wu_s, const void* Wd_s, void* ctx, void* stream);
+
 /* R1..R7: the whole forward.  X [T,H]; Wr [E,H]; bias [E] or NULL; Wg, Wu [E,F,H]; Wd [E,H,F];
  * shared expert Wg_s, Wu_s [F_shared,H], Wd_s [H,F_shared] or NULL (iff F_shared == 0).
- * Outputs Y [T,H], topk_idx [T,K], topk_w [T,K]; ctx receives what the backward needs. */
+ * Outputs Y [T,H], topk_idx [T,K], topk_w [T,K]; ctx receives what the backward needs.
+ * dtype 2 (R9): X, a are quantised 1x128 and the weights 128x128 on the fly (codes kept in ctx); Wg = Wu = Wd = NULL
+ * reuses the weight codes already in ctx; requires row_align % 128 == 0 and H, F, F_shared multiples of 128. */
 int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
                       const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
                       const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
@@ -141,7 +150,9 @@ int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, co
 
 /* R8: the whole backward for L = <Y, dY>.  Weight gradients are overwritten, in the weights' type.
  * Any of dWr / dWg / dWu / dWd (and the shared triple) may be NULL together with the others of its
- * group to skip the weight-gradient GEMMs (dX is always produced). */
+ * group to skip the weight-gradient GEMMs (dX is always produced).
+ * dtype 2 (R9): dgrad runs on e4m3 codes (Q(dY), Q(dg), Q(du), the weight codes in ctx; the bf16 weight pointers are
+ * not read and may be NULL), wgrad on the bf16 tensors. */
 int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const void* X, const void* Wr, const void* Wg,
                       const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
                       const void* ctx, void* dX, void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s,

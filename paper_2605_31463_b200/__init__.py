@@ -59,6 +59,7 @@ _SIGNATURES = {
     "moe_unpermute_combine": (_I32, [_CFG] + [_P] * 6),
     "moe_quantize_act": (_I32, [_P, _I64, _I32, _I32, _P, _P, _P]),
     "moe_quantize_weight": (_I32, [_P, _I32, _I32, _I32, _I32, _P, _P, _P]),
+    "moe_fp8_quantize_weights": (_I32, [_CFG] + [_P] * 8),
     "moe_layer_fwd": (_I32, [_CFG] + [_P] * 15),
     "moe_layer_bwd": (_I32, [_CFG] + [_P] * 20),
     "moe_layer_step_host": (_I32, [_CFG] + [_P] * 28),
@@ -211,6 +212,12 @@ def moe_quantize_act(v, rows, cols, scale_mode, codes, scales, stream=None):
 def moe_quantize_weight(w, batch, rows, cols, scale_mode, codes, scales, stream=None):
     _check(lib().moe_quantize_weight(_ptr(w), batch, rows, cols, scale_mode, _ptr(codes), _ptr(scales),
                                      _stream(stream)), "moe_quantize_weight")
+
+
+def moe_fp8_quantize_weights(cfg, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, stream=None):
+    _check(lib().moe_fp8_quantize_weights(C.byref(make_config(cfg)), _ptr(Wg), _ptr(Wu), _ptr(Wd), _ptr(Wg_s),
+                                          _ptr(Wu_s), _ptr(Wd_s), _ptr(ctx), _stream(stream)),
+           "moe_fp8_quantize_weights")
 
 
 def moe_layer_fwd(cfg, X, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, Y, topk_idx, topk_w, ctx, ws, stream=None):

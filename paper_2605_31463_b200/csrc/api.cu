@@ -1,6 +1,7 @@
 // Public grouped-GEMM entry points and the host-buffer step (include/moe_b200.h).
 #include <string.h>
 
+#include "fp8.cuh"
 #include "gemm_tc.cuh"
 
 using namespace moe;
@@ -12,8 +13,18 @@ extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int3
   MOE_CHECK(validate(cfg));
   cudaStream_t s = as_stream(stream);
   int32_t* mtile = reinterpret_cast<int32_t*>((char*)ws + ws_layout(cfg).tmp);
-  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;   // stand-alone fp8 GEMM: see fp8.cu
-  (void)a_scales; (void)b_scales;
+  if (cfg->dtype == 2) {   // e4m3 codes + block scales (R9)
+    if (!a_scales || !b_scales) return MOE_ERR_INVALID_ARG;
+    if (cfg->row_align % 128 != 0 || Kdim % 128 != 0 || N % 128 != 0) return MOE_ERR_UNSUPPORTED;
+    MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
+    F8Call c;
+    memset(&c, 0, sizeof(c));
+    c.mode = F8_FWD; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.mtile = mtile;
+    c.A = (const uint8_t*)A; c.lda = Kdim; c.a_scales = (const float*)a_scales;
+    c.B0 = (const uint8_t*)B; c.b0_scales = (const float*)b_scales; c.b_rows = N; c.b_cols = Kdim; c.N = N;
+    c.out0 = C; c.ld0 = N;
+    return fp8_gemm(c, s);
+  }
   if (cfg->dtype == 1 && cfg->row_align % 128 == 0 && Kdim % 64 == 0 && N % 8 == 0) {
     MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
     TcCall c;

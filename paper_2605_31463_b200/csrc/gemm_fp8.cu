@@ -1,0 +1,390 @@
+// FP8 e4m3 block-scaled grouped GEMM for sm_100a (SURVEY.md §8a a5/a6/a9/a11 in configs[3]; §8c R9).
+//
+// Persistent, warp-specialised: warp 0 = TMA producer, warp 1 = MMA issuer (tcgen05.mma kind::f8f6f4, M 128 x N 128
+// x K 32, four per 128-deep k-block), warps 2..9 = promotion + epilogue.  A k-block's partial product is written to
+// one of four 128-column TMEM buffers (never accumulated across k-blocks in TMEM); the promotion warps read it with
+// tcgen05.ld, multiply by sa[row, kb] * sb[n-block, kb] and add into fp32 register accumulators -- the block-scale
+// dequantisation of R9 fused into the main loop, exact up to fp32 rounding of the scaled sums.  Tiles are
+// 128 rows x 128 output columns, so every tile sees exactly one weight-scale scalar per k-block (two for the
+// gate/up pair of the fused SwiGLU forward, whose tile is 64 gate + 64 up columns).
+#include <string.h>
+
+#include <algorithm>
+
+#include "fp8.cuh"
+#include "tc_ptx.cuh"
+
+namespace moe {
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 128, UK = 32;
+constexpr int STAGES = 6;
+constexpr int A_BYTES = BM * BK, B_BYTES = BN * BK, STAGE_BYTES = A_BYTES + B_BYTES;   // 16 + 16 KB
+constexpr int NBUF = 4;                                                                  // TMEM partial-product ring
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int EPI_WARPS = 8;
+constexpr int NTHREADS = 64 + EPI_WARPS * 32;
+constexpr int TMEM_COLS = NBUF * BN;   // 512
+
+__device__ __forceinline__ void umma_f8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+
+struct F8Params {
+  int E, n_tiles, nkb, kb_split, b_rows, N, F;
+  int nb_b_cols;            // b_cols / 128 (scale row pitch of the weights)
+  int a_nblk;               // lda / 128 (scale row pitch of A)
+  int64_t rows_valid;
+  const int32_t* mtile;
+  const float* a_scales;
+  const float* b0_scales;
+  const float* b1_scales;
+  __nv_bfloat16* out0;
+  int64_t ld0;
+  __nv_bfloat16* out1;
+  int64_t ld1;
+  const __nv_bfloat16* gu;
+  int64_t ldgu;
+  const int32_t* p2f;
+  const float* w;
+};
+
+struct Tile {
+  int e, m0, n0;
+};
+
+template <int MODE>
+__device__ __forceinline__ bool decode_tile(const F8Params& p, int64_t t, int64_t total, Tile& tl) {
+  if (t >= total) return false;
+  const int mt = (int)(t / p.n_tiles);
+  tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == F8_FWD_SWIGLU ? BN / 2 : BN);
+  tl.m0 = mt * BM;
+  tl.e = p.mtile ? p.mtile[1 + mt] : 0;
+  return true;
+}
+
+__device__ __forceinline__ int64_t total_tiles(const F8Params& p) {
+  const int64_t mt = p.mtile ? p.mtile[0] : (p.rows_valid + BM - 1) / BM;
+  return mt * p.n_tiles;
+}
+
+// weight-scale scalar(s) of k-block kb for this tile.  K-major weights [E, N, Kd]: scales [E, N/128, Kd/128];
+// MN-major use (dgrad) of weights [E, b_rows, b_cols]: the contraction runs over b_rows, the output over b_cols.
+template <int MODE>
+__device__ __forceinline__ void weight_scales(const F8Params& p, const Tile& tl, int kb, float& s0, float& s1) {
+  if (MODE == F8_FWD) {
+    s0 = s1 = __ldg(p.b0_scales + ((int64_t)tl.e * (p.b_rows / 128) + tl.n0 / 128) * p.nb_b_cols + kb);
+  } else if (MODE == F8_FWD_SWIGLU) {
+    const int64_t i = ((int64_t)tl.e * (p.b_rows / 128) + tl.n0 / 128) * p.nb_b_cols + kb;
+    s0 = __ldg(p.b0_scales + i);
+    s1 = __ldg(p.b1_scales + i);
+  } else {
+    const bool second = kb >= p.kb_split;
+    const float* sc = second ? p.b1_scales : p.b0_scales;
+    const int kbl = second ? kb - p.kb_split : kb;
+    s0 = s1 = __ldg(sc + ((int64_t)tl.e * (p.b_rows / 128) + kbl) * p.nb_b_cols + tl.n0 / 128);
+  }
+}
+
+__device__ __forceinline__ uint4 pack8(const float* v) {
+  uint4 o;
+  o.x = pack_bf16(v[0], v[1]);
+  o.y = pack_bf16(v[2], v[3]);
+  o.z = pack_bf16(v[4], v[5]);
+  o.w = pack_bf16(v[6], v[7]);
+  return o;
+}
+
+__device__ __forceinline__ float fast_sigmoid8(float x) { return 1.0f / (1.0f + __expf(-x)); }
+
+// ---------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
+               const __grid_constant__ CUtensorMap tmB1, const F8Params p) {
+  constexpr bool B_MN = (MODE == F8_DGRAD || MODE == F8_DGRAD_SWIGLU);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = base + STAGES * STAGE_BYTES;
+  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, pfull0 = bars + 16 * STAGES, pempty0 = pfull0 + 8 * NBUF;
+  const uint32_t tmem_slot = pempty0 + 8 * NBUF;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB0);
+    tma_prefetch_desc(&tmB1);
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 1);
+    }
+    for (int b = 0; b < NBUF; ++b) {
+      mbar_init(pfull0 + 8 * b, 1);
+      mbar_init(pempty0 + 8 * b, EPI_WARPS);
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int64_t total = total_tiles(p);
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      Tile tl;
+      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+        for (int kb = 0; kb < p.nkb; ++kb) {
+          mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const uint32_t fb = full0 + 8 * stage;
+          const uint32_t sa = base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          mbar_expect_tx(fb, STAGE_BYTES);
+          tma_load_2d(sa, &tmA, fb, kb * BK, tl.m0);                                   // 128 B x 128 rows
+          if (MODE == F8_FWD) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);              // 128 B x 128 rows
+          } else if (MODE == F8_FWD_SWIGLU) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);              // 128 B x 64 rows (Wg)
+            tma_load_2d(sb + B_BYTES / 2, &tmB1, fb, kb * BK, tl.e * p.b_rows + tl.n0);  // (Wu)
+          } else {
+            const bool second = kb >= p.kb_split;
+            tma_load_2d(sb, second ? &tmB1 : &tmB0, fb, tl.n0,
+                        tl.e * p.b_rows + (second ? kb - p.kb_split : kb) * BK);       // 128 cols x 128 k-rows
+          }
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = instr_desc(0, 0, B_MN ? 1 : 0, BN);
+      int stage = 0, buf = 0;
+      uint32_t phase = 0, bphase = 0;
+      Tile tl;
+      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+        for (int kb = 0; kb < p.nkb; ++kb) {
+          mbar_wait(pempty0 + 8 * buf, bphase ^ 1);
+          mbar_wait(full0 + 8 * stage, phase);
+          tc_fence_after();
+          const uint32_t sa = base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          const uint32_t dacc = tmem_base + buf * BN;
+#pragma unroll
+          for (int k = 0; k < BK / UK; ++k) {
+            const uint64_t ad = smem_desc(sa + k * UK, 16, 1024);
+            const uint64_t bd = B_MN ? smem_desc(sb + k * UK * 128, B_BYTES, 1024) : smem_desc(sb + k * UK, 16, 1024);
+            umma_f8(dacc, ad, bd, idesc, k != 0);
+          }
+          umma_commit(empty0 + 8 * stage);
+          umma_commit(pfull0 + 8 * buf);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++buf == NBUF) { buf = 0; bphase ^= 1; }
+        }
+      }
+    }
+  } else {
+    // ===================== promotion + epilogue warps 2..9 =====================
+    const int lg = warp & 3;                   // TMEM lane group of this warp
+    const int ch = (warp - 2) >> 2;            // column half
+    const int row_in_tile = lg * 32 + lane;
+    const int c0 = (MODE == F8_FWD_SWIGLU) ? ch * 32 : ch * 64;
+    const int c1 = (MODE == F8_FWD_SWIGLU) ? 64 + ch * 32 : ch * 64 + 32;
+    int buf = 0;
+    uint32_t bphase = 0;
+    Tile tl;
+    for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      const int64_t row = (int64_t)tl.m0 + row_in_tile;
+      const bool row_ok = row < p.rows_valid;
+      const float* sa_row = p.a_scales + (row_ok ? row : 0) * p.a_nblk;
+      float acc0[32], acc1[32];
+#pragma unroll
+      for (int i = 0; i < 32; ++i) acc0[i] = acc1[i] = 0.f;
+      float sa_n = __ldg(sa_row), s0_n, s1_n;
+      weight_scales<MODE>(p, tl, 0, s0_n, s1_n);
+      for (int kb = 0; kb < p.nkb; ++kb) {
+        const float f0 = sa_n * s0_n, f1 = sa_n * s1_n;
+        if (kb + 1 < p.nkb) {
+          sa_n = __ldg(sa_row + kb + 1);
+          weight_scales<MODE>(p, tl, kb + 1, s0_n, s1_n);
+        }
+        mbar_wait(pfull0 + 8 * buf, bphase);
+        tc_fence_after();
+        const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + buf * BN;
+        uint32_t v0[32], v1[32];
+        tmem_ld32(tacc + c0, v0);
+        tmem_ld32(tacc + c1, v1);
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(pempty0 + 8 * buf);
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          acc0[i] = fmaf(f0, __uint_as_float(v0[i]), acc0[i]);
+          acc1[i] = fmaf(f1, __uint_as_float(v1[i]), acc1[i]);
+        }
+        if (++buf == NBUF) { buf = 0; bphase ^= 1; }
+      }
+      if (!row_ok) {
+        // rows past the buffer: nothing to store
+      } else if (MODE == F8_FWD || MODE == F8_DGRAD) {
+        __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          *reinterpret_cast<uint4*>(dst + c0 + q * 8) = pack8(acc0 + q * 8);
+          *reinterpret_cast<uint4*>(dst + c1 + q * 8) = pack8(acc1 + q * 8);
+        }
+      } else if (MODE == F8_FWD_SWIGLU) {
+        const int col = tl.n0 + ch * 32;
+        __nv_bfloat16* gdst = p.out0 + row * p.ld0 + col;
+        __nv_bfloat16* udst = gdst + p.F;
+        __nv_bfloat16* adst = p.out1 + row * p.ld1 + col;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          *reinterpret_cast<uint4*>(gdst + q * 8) = pack8(acc0 + q * 8);
+          *reinterpret_cast<uint4*>(udst + q * 8) = pack8(acc1 + q * 8);
+        }
+#pragma unroll
+        for (int i = 0; i < 32; ++i) acc0[i] = acc0[i] * fast_sigmoid8(acc0[i]) * acc1[i];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) *reinterpret_cast<uint4*>(adst + q * 8) = pack8(acc0 + q * 8);
+      } else {  // F8_DGRAD_SWIGLU
+        float rw = 1.0f;
+        if (p.w) {
+          const int pf = p.p2f[row];
+          rw = pf >= 0 ? p.w[pf] : 0.f;
+        }
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          const int col = tl.n0 + (half ? c1 : c0);
+          const float* acc = half ? acc1 : acc0;
+          const __nv_bfloat16* gsrc = p.gu + row * p.ldgu + col;
+          __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + col;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint4 gq = *reinterpret_cast<const uint4*>(gsrc + q * 8);
+            const uint4 uq = *reinterpret_cast<const uint4*>(gsrc + p.F + q * 8);
+            const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
+            float og[8], ou[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+              const float d0 = rw * acc[q * 8 + 2 * i], d1 = rw * acc[q * 8 + 2 * i + 1];
+              const float s0 = fast_sigmoid8(g0), s1 = fast_sigmoid8(g1);
+              og[2 * i] = d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0));
+              og[2 * i + 1] = d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1));
+              ou[2 * i] = d0 * g0 * s0;
+              ou[2 * i + 1] = d1 * g1 * s1;
+            }
+            *reinterpret_cast<uint4*>(dgdst + q * 8) = pack8(og);
+            *reinterpret_cast<uint4*>(dgdst + p.F + q * 8) = pack8(ou);
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host
+// ---------------------------------------------------------------------------------------------
+bool g_attr_set[4] = {false, false, false, false};
+
+template <int MODE>
+int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const F8Params& p, int64_t max_tiles,
+               cudaStream_t s) {
+  if (!g_attr_set[MODE]) {
+    MOE_CUDA(cudaFuncSetAttribute(f8_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    g_attr_set[MODE] = true;
+  }
+  const int sms = tc_sm_count();
+  if (sms <= 0) return MOE_ERR_CUDA;
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_tiles));
+  MOE_LAUNCH(f8_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, p);
+  return MOE_OK;
+}
+
+}  // namespace
+
+int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
+  if (c.mtile == nullptr && c.E != 1) return MOE_ERR_UNSUPPORTED;
+  if (!c.A || !c.a_scales || !c.B0 || !c.b0_scales || !c.out0) return MOE_ERR_INVALID_ARG;
+  if (c.lda % 128 || c.b_rows % 128 || c.b_cols % 128 || (c.ld0 & 7)) return MOE_ERR_UNSUPPORTED;
+  F8Params p;
+  memset(&p, 0, sizeof(p));
+  p.E = c.E;
+  p.rows_valid = c.rows_cap;
+  p.mtile = c.mtile;
+  p.a_scales = c.a_scales;
+  p.a_nblk = c.lda / 128;
+  p.b0_scales = c.b0_scales;
+  p.b1_scales = c.b1_scales ? c.b1_scales : c.b0_scales;
+  p.b_rows = c.b_rows;
+  p.nb_b_cols = c.b_cols / 128;
+  p.N = c.N;
+  p.F = c.F;
+  p.out0 = (__nv_bfloat16*)c.out0;
+  p.ld0 = c.ld0;
+  p.out1 = (__nv_bfloat16*)c.out1;
+  p.ld1 = c.ld1;
+  p.gu = (const __nv_bfloat16*)c.gu;
+  p.ldgu = c.ldgu;
+  p.p2f = c.p2f;
+  p.w = c.w;
+  CUtensorMap ta, tb0, tb1;
+  const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
+  const int64_t wrows = (int64_t)c.E * c.b_rows;
+  switch (c.mode) {
+    case F8_FWD: {
+      if (c.lda != c.b_cols || c.N != c.b_rows) return MOE_ERR_INVALID_ARG;
+      p.nkb = c.b_cols / BK;
+      p.n_tiles = c.N / BN;
+      if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, BN)) return MOE_ERR_UNSUPPORTED;
+      return launch<F8_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
+    }
+    case F8_FWD_SWIGLU: {
+      if (!c.B1 || !c.b1_scales || !c.out1 || c.lda != c.b_cols || c.F != c.b_rows || (c.ld1 & 7)) return MOE_ERR_INVALID_ARG;
+      p.nkb = c.b_cols / BK;
+      p.n_tiles = c.F / (BN / 2);
+      if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, BN / 2)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb1, 1, c.B1, c.b_cols, wrows, c.b_cols, BK, BN / 2)) return MOE_ERR_UNSUPPORTED;
+      return launch<F8_FWD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+    }
+    case F8_DGRAD:
+    case F8_DGRAD_SWIGLU: {
+      const bool split = c.B1 != nullptr;
+      if (c.N != c.b_cols || c.lda != (split ? 2 : 1) * c.b_rows) return MOE_ERR_INVALID_ARG;
+      p.kb_split = c.b_rows / BK;
+      p.nkb = split ? 2 * p.kb_split : p.kb_split;
+      p.n_tiles = c.N / BN;
+      if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb1, 1, split ? c.B1 : c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
+      if (c.mode == F8_DGRAD) return launch<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      if (!c.gu || c.F != c.b_cols || (c.ldgu & 7)) return MOE_ERR_INVALID_ARG;
+      return launch<F8_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+    }
+  }
+  return MOE_ERR_INVALID_ARG;
+}
+
+}  // namespace moe

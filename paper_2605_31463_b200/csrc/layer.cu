@@ -3,6 +3,7 @@
 // per-expert counts stay on the device.
 #include <string.h>
 
+#include "fp8.cuh"
 #include "gemm_tc.cuh"
 
 namespace moe {
@@ -114,6 +115,75 @@ int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* g
   return MOE_OK;
 }
 
+// Quantised operands of one FFN group on the fp8 path (R9): e4m3 codes + fp32 block scales.
+struct Fp8Bufs {
+  const uint8_t* Aq; const float* Aq_s;        // GEMM1 input rows [rows, H] (1x128)
+  uint8_t* aq; float* aq_s;                    // a [rows, F] (1x128)
+  const uint8_t *Wgq, *Wuq, *Wdq;              // weights (128x128)
+  const float *Wgq_s, *Wuq_s, *Wdq_s;
+  const uint8_t* dyq; const float* dyq_s;      // rows of Q(dY) [rows, H]
+  uint8_t* dguq; float* dguq_s;                // [dg|du] [rows, 2F]
+  const int32_t* p2f; const float* w;          // row weight of the dgrad-down epilogue (nullptr = 1)
+  int mode;
+};
+
+F8Call f8_base(const FfnGroup& g, int mode) {
+  F8Call c;
+  memset(&c, 0, sizeof(c));
+  c.mode = mode;
+  c.E = g.E;
+  c.rows_cap = g.rows_cap;
+  c.mtile = g.mtile;
+  c.F = g.F;
+  return c;
+}
+
+int32_t ffn_fwd_fp8(const FfnGroup& g, const Fp8Bufs& q, void* gu, void* a, void* y, cudaStream_t s) {
+  F8Call c = f8_base(g, F8_FWD_SWIGLU);   // gu = [Q(X) Q(Wg)^T | Q(X) Q(Wu)^T], a = silu(g) * u
+  c.A = q.Aq; c.lda = g.H; c.a_scales = q.Aq_s; c.B0 = q.Wgq; c.b0_scales = q.Wgq_s; c.B1 = q.Wuq; c.b1_scales = q.Wuq_s;
+  c.b_rows = g.F; c.b_cols = g.H; c.N = g.F; c.out0 = gu; c.ld0 = 2 * g.F; c.out1 = a; c.ld1 = g.F;
+  MOE_CHECK(fp8_gemm(c, s));
+  prof_mark(g.st_fwd1, s);
+  MOE_CHECK(fp8_quantize_act(a, g.rows_cap, g.F, q.mode, q.aq, q.aq_s, s));   // Q-a on the bf16 a
+  prof_mark(ST_QUANT, s);
+  c = f8_base(g, F8_FWD);                 // y = Q(a) Q(Wd)^T
+  c.A = q.aq; c.lda = g.F; c.a_scales = q.aq_s; c.B0 = q.Wdq; c.b0_scales = q.Wdq_s; c.b_rows = g.H; c.b_cols = g.F;
+  c.N = g.H; c.out0 = y; c.ld0 = g.H;
+  MOE_CHECK(fp8_gemm(c, s));
+  prof_mark(g.st_fwd2, s);
+  return MOE_OK;
+}
+
+// dgrad in fp8 (codes of dY rows, dg, du), wgrad in bf16 from dy, a, dgu, Xp (R9).
+int32_t ffn_bwd_fp8(const FfnGroup& g, const Fp8Bufs& q, const void* dy, const void* Xp, const void* gu, const void* a,
+                    void* dgu, void* dXp, void* dWg, void* dWu, void* dWd, cudaStream_t s) {
+  F8Call c = f8_base(g, F8_DGRAD_SWIGLU);  // dgu = swiglu'(gu) * w_r * (Q(dY)[t_r] Q(Wd)[e])
+  c.A = q.dyq; c.lda = g.H; c.a_scales = q.dyq_s; c.B0 = q.Wdq; c.b0_scales = q.Wdq_s; c.b_rows = g.H; c.b_cols = g.F;
+  c.N = g.F; c.gu = gu; c.ldgu = 2 * g.F; c.out0 = dgu; c.ld0 = 2 * g.F; c.p2f = q.p2f; c.w = q.w;
+  MOE_CHECK(fp8_gemm(c, s));
+  prof_mark(g.st_bwd1, s);
+  MOE_CHECK(fp8_quantize_act(dgu, g.rows_cap, 2 * g.F, q.mode, q.dguq, q.dguq_s, s));   // Q-dgu
+  prof_mark(ST_QUANT, s);
+  c = f8_base(g, F8_DGRAD);                // dXp = Q(dg) Q(Wg)[e] + Q(du) Q(Wu)[e]
+  c.A = q.dguq; c.lda = 2 * g.F; c.a_scales = q.dguq_s; c.B0 = q.Wgq; c.b0_scales = q.Wgq_s; c.B1 = q.Wuq;
+  c.b1_scales = q.Wuq_s; c.b_rows = g.F; c.b_cols = g.H; c.N = g.H; c.out0 = dXp; c.ld0 = g.H;
+  MOE_CHECK(fp8_gemm(c, s));
+  prof_mark(g.st_bwd2, s);
+  if (dWd) {
+    if (!(g.mtile != nullptr || g.E == 1)) return MOE_ERR_UNSUPPORTED;
+    TcCall t = tc_base(g, TC_WGRAD);
+    t.A = dy; t.lda = g.H; t.M = g.H; t.A2 = a; t.lda2 = g.F; t.N = g.F; t.out0 = dWd; t.ld0 = g.F;
+    MOE_CHECK(tc_gemm(t, s));
+    t = tc_base(g, TC_WGRAD);
+    t.A = dgu; t.lda = 2 * g.F; t.M = g.F; t.A2 = Xp; t.lda2 = g.H; t.N = g.H; t.out0 = dWg; t.ld0 = g.H;
+    MOE_CHECK(tc_gemm(t, s));
+    t.a_col0 = g.F; t.out0 = dWu;
+    MOE_CHECK(tc_gemm(t, s));
+    prof_mark(g.st_wgrad, s);
+  }
+  return MOE_OK;
+}
+
 template <typename T>
 T* at(const void* base, size_t off) {
   return reinterpret_cast<T*>((char*)base + off);
@@ -124,16 +194,43 @@ T* at(const void* base, size_t off) {
 
 using namespace moe;
 
+extern "C" int32_t moe_fp8_quantize_weights(const moe_config_t* cfg, const void* Wg, const void* Wu, const void* Wd,
+                                            const void* Wg_s, const void* Wu_s, const void* Wd_s, void* ctx,
+                                            void* stream) {
+  if (!cfg || !Wg || !Wu || !Wd || !ctx) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  if (cfg->dtype != 2) return MOE_ERR_INVALID_ARG;
+  const bool shared = cfg->F_shared > 0;
+  if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  cudaStream_t s = as_stream(stream);
+  const CtxLayout C = ctx_layout(cfg);
+  const int m = cfg->fp8_scale_mode, E = cfg->E, H = cfg->H, F = cfg->F, Fs = cfg->F_shared;
+  MOE_CHECK(fp8_quantize_weight(Wg, E, F, H, m, at<uint8_t>(ctx, C.Wgq), at<float>(ctx, C.Wgq_s), s));
+  MOE_CHECK(fp8_quantize_weight(Wu, E, F, H, m, at<uint8_t>(ctx, C.Wuq), at<float>(ctx, C.Wuq_s), s));
+  MOE_CHECK(fp8_quantize_weight(Wd, E, H, F, m, at<uint8_t>(ctx, C.Wdq), at<float>(ctx, C.Wdq_s), s));
+  if (shared) {
+    MOE_CHECK(fp8_quantize_weight(Wg_s, 1, Fs, H, m, at<uint8_t>(ctx, C.Wgsq), at<float>(ctx, C.Wgsq_s), s));
+    MOE_CHECK(fp8_quantize_weight(Wu_s, 1, Fs, H, m, at<uint8_t>(ctx, C.Wusq), at<float>(ctx, C.Wusq_s), s));
+    MOE_CHECK(fp8_quantize_weight(Wd_s, 1, H, Fs, m, at<uint8_t>(ctx, C.Wdsq), at<float>(ctx, C.Wdsq_s), s));
+  }
+  return MOE_OK;
+}
+
 extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
                                  const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
                                  const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
                                  void* stream) {
-  if (!cfg || !X || !Wr || !Wg || !Wu || !Wd || !Y || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
+  if (!cfg || !X || !Wr || !Y || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(validate(cfg));
   if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
   const bool shared = cfg->F_shared > 0;
-  if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
-  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;  // fp8 layer path: see layer_fp8.cu when present
+  const bool fp8 = cfg->dtype == 2;
+  // fp8: Wg == Wu == Wd == NULL means "use the e4m3 codes already in ctx" (the FP8 weight cache, PAPER.md:116,
+  // filled by an earlier moe_layer_fwd with weights or by moe_fp8_quantize_weights).
+  const bool cached = fp8 && !Wg && !Wu && !Wd;
+  if (!cached && (!Wg || !Wu || !Wd)) return MOE_ERR_INVALID_ARG;
+  if (shared && !cached && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  if (fp8 && cfg->row_align % 128 != 0) return MOE_ERR_UNSUPPORTED;
   cudaStream_t s = as_stream(stream);
   const CtxLayout C = ctx_layout(cfg);
   const WsLayout W = ws_layout(cfg);
@@ -162,14 +259,44 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
   FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
-  MOE_CHECK(ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s));                                      // R7
+  Fp8Bufs q, qs;
+  memset(&q, 0, sizeof(q));
+  memset(&qs, 0, sizeof(qs));
+  if (fp8) {                                                                               // R9 quantisation points
+    const int mode = cfg->fp8_scale_mode;
+    uint8_t* Xq = at<uint8_t>(ctx, C.Xq);
+    float* Xq_s = at<float>(ctx, C.Xq_s);
+    MOE_CHECK(fp8_quantize_act(X, cfg->T, cfg->H, mode, Xq, Xq_s, s));                     // Q-X once per token
+    MOE_CHECK(gather_rows(cfg, Xq, cfg->H, 1, f2p, p2f, offsets, at<uint8_t>(ctx, C.Xpq), s));
+    MOE_CHECK(fp8_gather_scales(Xq_s, p2f, offsets, cfg->E, cfg->K, cfg->H / 128, at<float>(ctx, C.Xpq_s), s));
+    if (!cached) MOE_CHECK(moe_fp8_quantize_weights(cfg, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, stream));   // Q-W
+    prof_mark(ST_QUANT, s);
+    q.Aq = at<uint8_t>(ctx, C.Xpq); q.Aq_s = at<float>(ctx, C.Xpq_s);
+    q.aq = at<uint8_t>(ctx, C.aq); q.aq_s = at<float>(ctx, C.aq_s);
+    q.Wgq = at<uint8_t>(ctx, C.Wgq); q.Wgq_s = at<float>(ctx, C.Wgq_s);
+    q.Wuq = at<uint8_t>(ctx, C.Wuq); q.Wuq_s = at<float>(ctx, C.Wuq_s);
+    q.Wdq = at<uint8_t>(ctx, C.Wdq); q.Wdq_s = at<float>(ctx, C.Wdq_s);
+    q.mode = mode;
+    qs = q;
+    qs.Aq = Xq; qs.Aq_s = Xq_s;
+    qs.aq = at<uint8_t>(ctx, C.asq); qs.aq_s = at<float>(ctx, C.asq_s);
+    qs.Wgq = at<uint8_t>(ctx, C.Wgsq); qs.Wgq_s = at<float>(ctx, C.Wgsq_s);
+    qs.Wuq = at<uint8_t>(ctx, C.Wusq); qs.Wuq_s = at<float>(ctx, C.Wusq_s);
+    qs.Wdq = at<uint8_t>(ctx, C.Wdsq); qs.Wdq_s = at<float>(ctx, C.Wdsq_s);
+    MOE_CHECK(ffn_fwd_fp8(g, q, gu, a, y, s));                                             // R7 on the codes
+  } else {
+    MOE_CHECK(ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s));                                    // R7
+  }
   const void* shared_out = nullptr;
   if (shared) {
     int32_t* off_s = offsets + cfg->E + 1;
     MOE_LAUNCH(set2_kernel, 1, 1, 0, s, off_s, 0, cfg->T);
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
-    MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
+    if (fp8)
+      MOE_CHECK(ffn_fwd_fp8(gs, qs, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
+    else
+      MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
     shared_out = at<char>(ctx, C.y_s);
   }
   MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, Y, s));    // R7 combine
@@ -181,15 +308,17 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
                                  const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
                                  const void* Wd_s, const void* ctx, void* dX, void* dWr, void* dWg, void* dWu,
                                  void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, void* ws, void* stream) {
-  if (!cfg || !dY || !X || !Wr || !Wg || !Wu || !Wd || !ctx || !dX || !ws) return MOE_ERR_INVALID_ARG;
+  if (!cfg || !dY || !X || !Wr || !ctx || !dX || !ws) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(validate(cfg));
   const bool shared = cfg->F_shared > 0;
-  if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  const bool fp8 = cfg->dtype == 2;   // fp8: the dgrad reads the codes saved in ctx; the bf16 weights are not touched
+  if (!fp8 && (!Wg || !Wu || !Wd)) return MOE_ERR_INVALID_ARG;
+  if (!fp8 && shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  if (fp8 && cfg->row_align % 128 != 0) return MOE_ERR_UNSUPPORTED;
   const bool wgrad = dWg || dWu || dWd;
   if (wgrad && !(dWg && dWu && dWd)) return MOE_ERR_INVALID_ARG;
   const bool wgrad_s = dWg_s || dWu_s || dWd_s;
   if (wgrad_s && !(shared && dWg_s && dWu_s && dWd_s)) return MOE_ERR_INVALID_ARG;
-  if (cfg->dtype == 2) return MOE_ERR_UNSUPPORTED;
   cudaStream_t s = as_stream(stream);
   const CtxLayout C = ctx_layout(cfg);
   const WsLayout W = ws_layout(cfg);
@@ -219,7 +348,34 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
-  MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));       // R8 expert FFN
+  Fp8Bufs q, qs;
+  memset(&q, 0, sizeof(q));
+  memset(&qs, 0, sizeof(qs));
+  if (fp8) {
+    const int mode = cfg->fp8_scale_mode;
+    uint8_t* dYq = at<uint8_t>(ws, W.dYq);
+    float* dYq_s = at<float>(ws, W.dYq_s);
+    MOE_CHECK(fp8_quantize_act(dY, cfg->T, cfg->H, mode, dYq, dYq_s, s));                  // Q-dY (w applied after the GEMM)
+    MOE_CHECK(gather_rows(cfg, dYq, cfg->H, 1, f2p, p2f, offsets, at<uint8_t>(ws, W.dyq), s));
+    MOE_CHECK(fp8_gather_scales(dYq_s, p2f, offsets, cfg->E, cfg->K, cfg->H / 128, at<float>(ws, W.dyq_s), s));
+    prof_mark(ST_QUANT, s);
+    q.Wgq = at<uint8_t>(ctx, C.Wgq); q.Wgq_s = at<float>(ctx, C.Wgq_s);
+    q.Wuq = at<uint8_t>(ctx, C.Wuq); q.Wuq_s = at<float>(ctx, C.Wuq_s);
+    q.Wdq = at<uint8_t>(ctx, C.Wdq); q.Wdq_s = at<float>(ctx, C.Wdq_s);
+    q.dyq = at<uint8_t>(ws, W.dyq); q.dyq_s = at<float>(ws, W.dyq_s);
+    q.dguq = at<uint8_t>(ws, W.dguq); q.dguq_s = at<float>(ws, W.dguq_s);
+    q.p2f = p2f; q.w = w; q.mode = mode;
+    qs = q;
+    qs.Wgq = at<uint8_t>(ctx, C.Wgsq); qs.Wgq_s = at<float>(ctx, C.Wgsq_s);
+    qs.Wuq = at<uint8_t>(ctx, C.Wusq); qs.Wuq_s = at<float>(ctx, C.Wusq_s);
+    qs.Wdq = at<uint8_t>(ctx, C.Wdsq); qs.Wdq_s = at<float>(ctx, C.Wdsq_s);
+    qs.dyq = dYq; qs.dyq_s = dYq_s;
+    qs.dguq = at<uint8_t>(ws, W.dgusq); qs.dguq_s = at<float>(ws, W.dgusq_s);
+    qs.p2f = nullptr; qs.w = nullptr;
+    MOE_CHECK(ffn_bwd_fp8(g, q, dy, Xp, gu, a, dgu, dXp, dWg, dWu, dWd, s));               // R8 expert FFN on the codes
+  } else {
+    MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));     // R8 expert FFN
+  }
   MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, Xp, dz, dzp, dWr, s));    // R8 router
   prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
@@ -227,8 +383,12 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
     const int32_t* off_s = offsets + cfg->E + 1;
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
-    MOE_CHECK(ffn_bwd(gs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), Wg_s, Wu_s, Wd_s, tmp,
-                      at<char>(ws, W.dgu_s), at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
+    if (fp8)
+      MOE_CHECK(ffn_bwd_fp8(gs, qs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ws, W.dgu_s),
+                            at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
+    else
+      MOE_CHECK(ffn_bwd(gs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), Wg_s, Wu_s, Wd_s, tmp,
+                        at<char>(ws, W.dgu_s), at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
     dXs = at<char>(ws, W.dXs);
   }
   // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]
