@@ -348,6 +348,31 @@ def fq_weight(w, mode):
     return dequantize_128x128(c, s)
 
 
+def expert_ffn_fwd_fp8(Xq, Wg, Wu, Wd, mode):
+    """R9 forward of one expert: Xq = dequantised Q-X rows (fp64); weights bf16-grid, fake-quantised 128x128 here;
+    a is bf16-rounded and fake-quantised 1x128 before the down projection (Q-a)."""
+    Wgq, Wuq, Wdq = fq_weight(Wg, mode), fq_weight(Wu, mode), fq_weight(Wd, mode)
+    g = Xq @ Wgq.T
+    u = Xq @ Wuq.T
+    a = swiglu(g, u)
+    y = fq_act(a, mode) @ Wdq.T
+    return g, u, a, y
+
+
+def expert_ffn_bwd_fp8(dYq, wr, dy, Xb, g, u, a, Wg, Wu, Wd, mode):
+    """R9 backward of one expert.  dYq = dequantised Q-dY rows of the expert's tokens, wr = their gating weights
+    (applied after the GEMM), dy = wr*dY (bf16 tensor of the wgrad), Xb = the bf16 input rows.  dgrad on
+    fake-quantised operands (Q-dY, Q-dgu, Q-W); wgrad on the bf16-rounded tensors."""
+    Wgq, Wuq, Wdq = fq_weight(Wg, mode), fq_weight(Wu, mode), fq_weight(Wd, mode)
+    da = np.asarray(wr, F64)[:, None] * (dYq @ Wdq)
+    dg, du = swiglu_bwd(da, g, u)
+    dX = fq_act(dg, mode) @ Wgq + fq_act(du, mode) @ Wuq
+    dWd = np.asarray(bf16_round(dy), F64).T @ np.asarray(bf16_round(a), F64)
+    dWg = np.asarray(bf16_round(dg), F64).T @ Xb
+    dWu = np.asarray(bf16_round(du), F64).T @ Xb
+    return dX, dWg, dWu, dWd, dg, du
+
+
 # =====================================================================================
 # whole layer, forward and backward (R1..R9)
 # =====================================================================================
@@ -379,20 +404,14 @@ def layer_fwd(cfg, X, Wr, bias, W, shared=None, forced_idx=None, key_dtype=F64):
             continue
         Wg, Wu, Wd = _expert_weights(W, e)
         if fp8:
-            Wg, Wu, Wd = fq_weight(Wg, mode), fq_weight(Wu, mode), fq_weight(Wd, mode)
-            ge = Xp[lo:lo + c] @ Wg.T
-            ue = Xp[lo:lo + c] @ Wu.T
-            ae = swiglu(ge, ue)
-            ye = fq_act(ae, mode) @ Wd.T                      # Q-a on the bf16-rounded a
+            ge, ue, ae, ye = expert_ffn_fwd_fp8(Xp[lo:lo + c], Wg, Wu, Wd, mode)
         else:
             ge, ue, ae, ye = expert_ffn_fwd(Xp[lo:lo + c], Wg, Wu, Wd)
         g[lo:lo + c], u[lo:lo + c], a[lo:lo + c], y[lo:lo + c] = ge, ue, ae, ye
     sh = None
     if shared is not None:
         if fp8:
-            sWg, sWu, sWd = (fq_weight(s_, mode) for s_ in shared)
-            sg = Xin @ sWg.T; su = Xin @ sWu.T; sa = swiglu(sg, su)
-            sy = fq_act(sa, mode) @ sWd.T
+            sg, su, sa, sy = expert_ffn_fwd_fp8(Xin, *shared, mode)
         else:
             sg, su, sa, sy = expert_ffn_fwd(X, *shared)
         sh = dict(g=sg, u=su, a=sa, y=sy)
@@ -469,13 +488,8 @@ def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None):
         sl = slice(lo, lo + c)
         Wg, Wu, Wd = _expert_weights(W, e)
         if fp8:
-            Wgq, Wuq, Wdq = fq_weight(Wg, mode), fq_weight(Wu, mode), fq_weight(Wd, mode)
-            da = wr[sl, None] * (dYq[tok[sl]] @ Wdq)
-            dg, du = swiglu_bwd(da, fwd["g"][sl], fwd["u"][sl])
-            dXp[sl] = fq_act(dg, mode) @ Wgq + fq_act(du, mode) @ Wuq           # Q-dgu
-            dWd[e] = np.asarray(bf16_round(dy[sl]), F64).T @ np.asarray(bf16_round(fwd["a"][sl]), F64)
-            dWg[e] = np.asarray(bf16_round(dg), F64).T @ Xpb[sl]
-            dWu[e] = np.asarray(bf16_round(du), F64).T @ Xpb[sl]
+            dXp[sl], dWg[e], dWu[e], dWd[e], dg, du = expert_ffn_bwd_fp8(
+                dYq[tok[sl]], wr[sl], dy[sl], Xpb[sl], fwd["g"][sl], fwd["u"][sl], fwd["a"][sl], Wg, Wu, Wd, mode)
         else:
             dXp[sl], dWg[e], dWu[e], dWd[e], dg, du = expert_ffn_bwd(
                 dy[sl], Xpb[sl], fwd["g"][sl], fwd["u"][sl], fwd["a"][sl], Wg, Wu, Wd)
@@ -489,13 +503,8 @@ def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None):
     if shared is not None:
         sh = fwd["shared"]
         if fp8:
-            sWg, sWu, sWd = (fq_weight(s_, mode) for s_ in shared)
-            da = dYq @ sWd
-            dg, du = swiglu_bwd(da, sh["g"], sh["u"])
-            dXs = fq_act(dg, mode) @ sWg + fq_act(du, mode) @ sWu
-            out["dWd_s"] = dY.T @ np.asarray(bf16_round(sh["a"]), F64)
-            out["dWg_s"] = np.asarray(bf16_round(dg), F64).T @ X64
-            out["dWu_s"] = np.asarray(bf16_round(du), F64).T @ X64
+            dXs, out["dWg_s"], out["dWu_s"], out["dWd_s"], _, _ = expert_ffn_bwd_fp8(
+                dYq, np.ones(T, F64), dY, X64, sh["g"], sh["u"], sh["a"], *shared, mode)
         else:
             dXs, out["dWg_s"], out["dWu_s"], out["dWd_s"], _, _ = expert_ffn_bwd(
                 dY, X64, sh["g"], sh["u"], sh["a"], *shared)
