@@ -52,7 +52,7 @@ def pick_config(name):
 # the oracle leg (cpu_baseline and --impl reference): a bounded sample of the same workload
 # ----------------------------------------------------------------------------------------------------
 
-def oracle_sample(cfg, budget_s=12.0, max_experts=24):
+def oracle_sample(cfg, budget_s=15.0, max_experts=None):
     """Oracle routing over all T tokens, then the oracle's expert FFN fwd+bwd (fp64) for experts 0..n-1 on the
     rows routed to them, until `budget_s` of CPU time is spent.  Returns (flops, seconds, description)."""
     from oracle import moe_oracle as orc
@@ -65,7 +65,7 @@ def oracle_sample(cfg, budget_s=12.0, max_experts=24):
     t_route = time.perf_counter() - t0
     flops = 2.0 * cfg.T * cfg.H * cfg.E
     spent, n, rows = t_route, 0, 0
-    for e in range(min(cfg.E, max_experts)):
+    for e in range(cfg.E if max_experts is None else min(cfg.E, max_experts)):
         Wg, Wu, Wd = wl.gen_expert_weights(cfg, e)            # generation is not timed
         r0, r1 = int(offsets[e]), int(offsets[e]) + int(counts[e])
         if r1 == r0:

@@ -66,7 +66,7 @@ struct CtxLayout {
   size_t total;
 };
 struct WsLayout {
-  size_t hist, tmp, dw, dz, dzp, dy, dgu, dXp, dgu_s, dXs, dYq, dYq_s, dyq, dyq_s, dguq, dguq_s, dgusq, dgusq_s;
+  size_t hist, tmp, dw, dz, dzp, dwr_part, dy, dgu, dXp, dgu_s, dXs, dYq, dYq_s, dyq, dyq_s, dguq, dguq_s, dgusq, dgusq_s;
   size_t total;
 };
 CtxLayout ctx_layout(const moe_config_t* c);
@@ -87,8 +87,8 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
 // router.cu
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s);
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
-                   const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const void* Xp, float* dz,
-                   float* dzp, void* dWr, cudaStream_t s);
+                   const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const int32_t* mtile,
+                   const void* Xp, float* dz, float* dzp, float* part, void* dWr, cudaStream_t s);
 // gemm_simt.cu: reference-free fallback GEMMs for fp32 (and any shape the tensor-core path rejects)
 //   mode 0: C[r,n]    = sum_k A[r,k] B[e][n,k]           (rows grouped by offsets)
 //   mode 1: dA[r,k]   = sum_n dC[r,n] B[e][n,k]

@@ -58,6 +58,19 @@ bool tc_make_map(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t inner,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+bool tc_make_map3(CUtensorMap* m, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0, int box1) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn || !ptr || d0 <= 0 || d1 <= 0 || d2 <= 0) return false;
+  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || ((ld * 2) & 15)) return false;
+  const cuuint64_t dims[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * 2, (cuuint64_t)d1 * ld * 2};
+  const cuuint32_t box[3] = {(cuuint32_t)box0, (cuuint32_t)box1, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 int tc_sm_count() {
   static int n = 0;
   if (n == 0) {
@@ -78,8 +91,10 @@ constexpr int A_BYTES = BM * BK * 2;   // 16 KB
 constexpr int B_BYTES = BN * BK * 2;   // 32 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int MN_BOX_BYTES = 64 * BK * 2;  // one 64(MN) x 64(K) box of an MN-major operand: 8 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
-constexpr int NTHREADS = 192;
+constexpr int OBUF_BYTES = BM * 128;       // epilogue staging: 128 rows x 64 bf16 columns (one 128-byte-swizzled TMA box)
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * OBUF_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int EPI_WARPS = 8;            // two per TMEM lane group: column-chunk parity `ch` splits a tile between them
+constexpr int NTHREADS = 64 + EPI_WARPS * 32;
 constexpr int TMEM_COLS = 512;
 
 // ---------------------------------------------------------------------------------------------
@@ -154,18 +169,18 @@ __device__ __forceinline__ void store_row_chunk(__nv_bfloat16* dst, const uint32
   }
 }
 
-__device__ __forceinline__ float fast_sigmoid(float x) { return 1.0f / (1.0f + __expf(-x)); }
+__device__ __forceinline__ float fast_sigmoid(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
 template <int MODE>
 __device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
-                                              bool have_acc) {
+                                              bool have_acc, int ch) {
   // tacc: TMEM address of this warp's lane group at the accumulator stage's first column
   if (MODE == TC_FWD || MODE == TC_DGRAD) {
     const int64_t row = (int64_t)tl.m0 + row_in_tile;
     const bool row_ok = row < p.rows_valid;
     __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0;
 #pragma unroll 1
-    for (int c = 0; c < BN / 32; ++c) {
+    for (int c = ch; c < BN / 32; c += 2) {
       const int ncols = p.N - (tl.n0 + c * 32);   // warp-uniform
       if (ncols <= 0) break;
       uint32_t v[32];
@@ -173,23 +188,23 @@ __device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl,
       tmem_ld_wait();
       if (row_ok) store_row_chunk(dst + c * 32, v, ncols);
     }
-  } else if (MODE == TC_WGRAD) {
-    const int m = tl.m0 + row_in_tile;
-    const bool row_ok = m < p.M;
-    __nv_bfloat16* dst = p.out0 + ((int64_t)tl.e * p.M + m) * p.ld0 + tl.n0;
+  } else if (MODE == TC_FWD_F32) {
+    const int64_t row = (int64_t)tl.m0 + row_in_tile;
+    const bool row_ok = row < p.rows_valid;
+    float* dst = reinterpret_cast<float*>(p.out0) + row * p.ld0 + tl.n0;
 #pragma unroll 1
-    for (int c = 0; c < BN / 32; ++c) {
-      const int ncols = p.N - (tl.n0 + c * 32);
+    for (int c = ch; c < BN / 32; c += 2) {
+      const int ncols = p.N - (tl.n0 + c * 32);   // warp-uniform, multiple of 4
       if (ncols <= 0) break;
       uint32_t v[32];
-      if (have_acc) {
-        tmem_ld32(tacc + c * 32, v);
-        tmem_ld_wait();
-      } else {
+      tmem_ld32(tacc + c * 32, v);
+      tmem_ld_wait();
+      if (row_ok) {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) v[i] = 0u;   // empty expert: exact zeros
+        for (int q = 0; q < 8; ++q)
+          if (q * 4 < ncols)
+            *reinterpret_cast<uint4*>(dst + c * 32 + q * 4) = make_uint4(v[q * 4], v[q * 4 + 1], v[q * 4 + 2], v[q * 4 + 3]);
       }
-      if (row_ok) store_row_chunk(dst + c * 32, v, ncols);
     }
   } else if (MODE == TC_FWD_SWIGLU) {
     // accumulator columns [0,128) = gate, [128,256) = up for output columns n0 .. n0+127
@@ -199,7 +214,7 @@ __device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl,
     __nv_bfloat16* udst = gdst + p.F;
     __nv_bfloat16* adst = p.out1 + row * p.ld1 + tl.n0;
 #pragma unroll 1
-    for (int c = 0; c < BN / 64; ++c) {
+    for (int c = ch; c < BN / 64; c += 2) {
       const int ncols = p.F - (tl.n0 + c * 32);
       if (ncols <= 0) break;
       uint32_t g[32], u[32];
@@ -217,39 +232,98 @@ __device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl,
       }
       if (row_ok) store_row_chunk(adst + c * 32, g, ncols);
     }
-  } else {  // TC_DGRAD_SWIGLU: acc = da [128 x 256 columns of F]
-    const int64_t row = (int64_t)tl.m0 + row_in_tile;
-    const bool row_ok = row < p.rows_valid;
-    const __nv_bfloat16* gsrc = p.gu + row * p.ldgu + tl.n0;
-    __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + tl.n0;
-#pragma unroll 1
-    for (int c = 0; c < BN / 32; ++c) {
-      const int ncols = p.F - (tl.n0 + c * 32);
-      if (ncols <= 0) break;
-      uint32_t d[32];
-      tmem_ld32(tacc + c * 32, d);
-      tmem_ld_wait();
-      if (row_ok) {
+  }
+}
+
+// TC_DGRAD_SWIGLU epilogue: acc = da [128 x 256 columns of F]; dgu = swiglu'(g, u) * da.  The saved g, u of this
+// thread's row are fetched from HBM two 32-column chunks ahead of the TMEM drain (the first two before the
+// accumulator is even complete), so their latency hides behind the main loop and the previous chunk's math.
+struct GuChunk {
+  uint4 g[4], u[4];
+};
+
+__device__ __forceinline__ void gu_load(const TcParams& p, const Tile& tl, int64_t row, bool row_ok, int c, GuChunk& k) {
+  const int ncols = p.F - (tl.n0 + c * 32);
+  if (!row_ok || ncols <= 0) return;
+  const uint4* gp = reinterpret_cast<const uint4*>(p.gu + row * p.ldgu + tl.n0 + c * 32);
+  const uint4* up = reinterpret_cast<const uint4*>(p.gu + row * p.ldgu + p.F + tl.n0 + c * 32);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          if (q * 8 < ncols) {
-            const uint4 gq = *reinterpret_cast<const uint4*>(gsrc + c * 32 + q * 8);
-            const uint4 uq = *reinterpret_cast<const uint4*>(gsrc + p.F + c * 32 + q * 8);
-            const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
-            uint32_t og[4], ou[4];
+  for (int q = 0; q < 4; ++q)
+    if (q * 8 < ncols) {
+      k.g[q] = __ldg(gp + q);
+      k.u[q] = __ldg(up + q);
+    }
+}
+
+__device__ __forceinline__ void dgrad_swiglu_chunk(const TcParams& p, const Tile& tl, int64_t row, bool row_ok, int c,
+                                                   uint32_t tacc, const GuChunk& k) {
+  const int ncols = p.F - (tl.n0 + c * 32);   // warp-uniform
+  if (ncols <= 0) return;
+  uint32_t d[32];
+  tmem_ld32(tacc + c * 32, d);
+  tmem_ld_wait();
+  if (!row_ok) return;
+  __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + tl.n0 + c * 32;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
-              const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
-              const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
-              og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
-              ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
-            }
-            *reinterpret_cast<uint4*>(dgdst + c * 32 + q * 8) = make_uint4(og[0], og[1], og[2], og[3]);
-            *reinterpret_cast<uint4*>(dgdst + p.F + c * 32 + q * 8) = make_uint4(ou[0], ou[1], ou[2], ou[3]);
-          }
-        }
+  for (int q = 0; q < 4; ++q) {
+    if (q * 8 < ncols) {
+      const uint32_t gw[4] = {k.g[q].x, k.g[q].y, k.g[q].z, k.g[q].w}, uw[4] = {k.u[q].x, k.u[q].y, k.u[q].z, k.u[q].w};
+      uint32_t og[4], ou[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+        const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
+        const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
+        og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
+        ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
       }
+      *reinterpret_cast<uint4*>(dgdst + q * 8) = make_uint4(og[0], og[1], og[2], og[3]);
+      *reinterpret_cast<uint4*>(dgdst + p.F + q * 8) = make_uint4(ou[0], ou[1], ou[2], ou[3]);
+    }
+  }
+}
+
+// TC_WGRAD epilogue.  An expert's contraction is short (its row count), so the weight-gradient tiles are bound by
+// how fast 128 x 256 bf16 outputs leave the SM: each 64-column chunk is packed into a 128-byte-swizzled shared-memory
+// box (thread = row, conflict-free 16-byte stores) and written with one TMA store (full 128-byte lines; rows past M
+// and columns past N are clipped by the 3-D tensor map [E, M, N]).  The two column-parity warp groups own one box each
+// and alternate, so one group's TMA store overlaps the other group's TMEM drain.
+__device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
+                                                 bool have_acc, uint32_t obuf, const CUtensorMap* tmO, bool issuer,
+                                                 int ch) {
+#pragma unroll 1
+  for (int c = ch; c < BN / 64; c += 2) {
+    const int ncols = p.N - (tl.n0 + c * 64);   // warp-uniform
+    if (ncols <= 0) break;
+    uint32_t v0[32], v1[32];
+    if (have_acc) {
+      tmem_ld32(tacc + c * 64, v0);
+      tmem_ld32(tacc + c * 64 + 32, v1);
+      tmem_ld_wait();
+    } else {
+#pragma unroll
+      for (int i = 0; i < 32; ++i) v0[i] = v1[i] = 0u;   // empty expert: exact zeros
+    }
+    if (issuer) bulk_wait_read0();     // this group's previous TMA store has finished reading the box
+    named_bar_sync(1 + ch, 128);
+    const uint32_t rowaddr = obuf + row_in_tile * 128;
+    const int sw = row_in_tile & 7;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      st_shared_v4(rowaddr + ((j ^ sw) << 4), pack_bf16(__uint_as_float(v0[j * 8 + 0]), __uint_as_float(v0[j * 8 + 1])),
+                   pack_bf16(__uint_as_float(v0[j * 8 + 2]), __uint_as_float(v0[j * 8 + 3])),
+                   pack_bf16(__uint_as_float(v0[j * 8 + 4]), __uint_as_float(v0[j * 8 + 5])),
+                   pack_bf16(__uint_as_float(v0[j * 8 + 6]), __uint_as_float(v0[j * 8 + 7])));
+      st_shared_v4(rowaddr + (((j + 4) ^ sw) << 4), pack_bf16(__uint_as_float(v1[j * 8 + 0]), __uint_as_float(v1[j * 8 + 1])),
+                   pack_bf16(__uint_as_float(v1[j * 8 + 2]), __uint_as_float(v1[j * 8 + 3])),
+                   pack_bf16(__uint_as_float(v1[j * 8 + 4]), __uint_as_float(v1[j * 8 + 5])),
+                   pack_bf16(__uint_as_float(v1[j * 8 + 6]), __uint_as_float(v1[j * 8 + 7])));
+    }
+    fence_proxy_async();
+    named_bar_sync(1 + ch, 128);
+    if (issuer) {
+      tma_store_3d(tmO, obuf, tl.n0 + c * 64, tl.m0, tl.e);
+      bulk_commit();
     }
   }
 }
@@ -265,7 +339,8 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128-byte swizzle wants 1024-byte alignment
-  const uint32_t bars = base + STAGES * STAGE_BYTES;
+  const uint32_t obuf0 = base + STAGES * STAGE_BYTES;
+  const uint32_t bars = obuf0 + 2 * OBUF_BYTES;
   // barrier addresses: full[s] = bars + 8 s; empty[s] = bars + 8 (STAGES + s); tfull[a] / tempty[a] follow
   const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
   const uint32_t tmem_slot = tempty0 + 16;
@@ -281,7 +356,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull0 + 8 * a, 1);
-      mbar_init(tempty0 + 8 * a, 4);   // one arrive per epilogue warp
+      mbar_init(tempty0 + 8 * a, EPI_WARPS);   // one arrive per epilogue warp
     }
     fence_barrier_init();
   }
@@ -313,7 +388,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
             for (int i = 0; i < BM / 64; ++i) tma_load_2d(sa + i * MN_BOX_BYTES, &tmA, fb, p.a_col0 + tl.m0 + 64 * i, kr);
           }
-          if (MODE == TC_FWD) {
+          if (MODE == TC_FWD || MODE == TC_FWD_F32) {
             tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 256
           } else if (MODE == TC_FWD_SWIGLU) {
             tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 128 (Wg)
@@ -365,18 +440,40 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   } else {
     // ===================== epilogue warps 2..5 =====================
     const int lg = warp & 3;                 // TMEM lane group this warp may access
+    const int ch = (warp - 2) >> 2;          // which half of the column chunks this warp drains
     const int row_in_tile = lg * 32 + lane;
     int as = 0;
     uint32_t aphase = 0;
     Tile tl;
     for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
       const bool have = tl.nkb > 0;
-      if (have) {
+      const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + as * BN;
+      if (MODE == TC_DGRAD_SWIGLU) {
+        const int64_t row = (int64_t)tl.m0 + row_in_tile;
+        const bool row_ok = row < p.rows_valid;
+        GuChunk k[3];
+        gu_load(p, tl, row, row_ok, ch, k[0]);
+        gu_load(p, tl, row, row_ok, ch + 2, k[1]);
         mbar_wait(tfull0 + 8 * as, aphase);
         tc_fence_after();
+#pragma unroll
+        for (int i = 0; i < BN / 64; ++i) {      // this warp's chunks: c = ch, ch + 2, ...
+          if (i + 2 < BN / 64) gu_load(p, tl, row, row_ok, ch + 2 * (i + 2), k[(i + 2) % 3]);
+          dgrad_swiglu_chunk(p, tl, row, row_ok, ch + 2 * i, tacc, k[i % 3]);
+        }
+      } else if (MODE == TC_WGRAD) {
+        if (have) {
+          mbar_wait(tfull0 + 8 * as, aphase);
+          tc_fence_after();
+        }
+        wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmB1, (threadIdx.x & 127) == 64, ch);
+      } else {
+        if (have) {
+          mbar_wait(tfull0 + 8 * as, aphase);
+          tc_fence_after();
+        }
+        epilogue_tile<MODE>(p, tl, tacc, row_in_tile, have, ch);
       }
-      const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + as * BN;
-      epilogue_tile<MODE>(p, tl, tacc, row_in_tile, have);
       if (have) {
         tc_fence_before();
         __syncwarp();
@@ -384,6 +481,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
+    if (MODE == TC_WGRAD && (threadIdx.x & 127) == 64) bulk_wait0();   // all TMA stores complete before the CTA retires
   }
   tc_fence_before();
   __syncthreads();
@@ -400,7 +498,7 @@ bool make_map(CUtensorMap* m, const void* ptr, int64_t inner, int64_t outer, int
 }
 
 int g_sm_count = 0;
-bool g_attr_set[5] = {false, false, false, false, false};
+bool g_attr_set[6] = {false, false, false, false, false, false};
 
 template <int MODE>
 int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const TcParams& p, int64_t max_tiles,
@@ -457,14 +555,16 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.a_col0 = c.a_col0;
   CUtensorMap ta, tb0, tb1;
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
-  if ((c.N & 7) || (c.ld0 & 7)) return MOE_ERR_UNSUPPORTED;
+  if (c.mode == TC_FWD_F32 ? ((c.N & 3) || (c.ld0 & 3)) : ((c.N & 7) || (c.ld0 & 7))) return MOE_ERR_UNSUPPORTED;
   switch (c.mode) {
+    case TC_FWD_F32:
     case TC_FWD: {
       if (c.Kd % BK) return MOE_ERR_UNSUPPORTED;
       p.nkb = c.Kd / BK;
       p.n_tiles = (int)ceil_div(c.N, BN);
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
+      if (c.mode == TC_FWD_F32) return launch<TC_FWD_F32>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
       return launch<TC_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
     }
     case TC_FWD_SWIGLU: {
@@ -497,7 +597,8 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       // A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (inner = output columns)
       if (!make_map(&ta, c.A, c.lda, c.rows_cap, c.lda, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.A2, c.N, c.rows_cap, c.lda2, 64)) return MOE_ERR_UNSUPPORTED;
-      return launch<TC_WGRAD>(ta, tb0, tb0, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
+      if (!tc_make_map3(&tb1, c.out0, c.N, c.M, c.E, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dB [E, M, N]
+      return launch<TC_WGRAD>(ta, tb0, tb1, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
     }
   }
   return MOE_ERR_INVALID_ARG;

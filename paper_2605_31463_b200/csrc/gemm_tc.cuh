@@ -12,7 +12,8 @@ namespace moe {
 //  TC_DGRAD_SWIGLU da = dy Wd[e]; dgu = swiglu'(gu) * da                                   (R8)
 //  TC_WGRAD        dB[e][n,k]  = sum_{r in e} dC[r,n] A[r,k]            both operands MN-major, the contraction
 //                  length is the expert's (padded) row count; an empty expert gets zeros   (R8)
-enum TcMode { TC_FWD = 0, TC_FWD_SWIGLU = 1, TC_DGRAD = 2, TC_DGRAD_SWIGLU = 3, TC_WGRAD = 4 };
+//  TC_FWD_F32      as TC_FWD with fp32 output (router logits z = X Wr^T, R1)
+enum TcMode { TC_FWD = 0, TC_FWD_SWIGLU = 1, TC_DGRAD = 2, TC_DGRAD_SWIGLU = 3, TC_WGRAD = 4, TC_FWD_F32 = 5 };
 
 struct TcCall {
   int mode;

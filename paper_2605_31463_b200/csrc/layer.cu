@@ -376,7 +376,8 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   } else {
     MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));     // R8 expert FFN
   }
-  MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, Xp, dz, dzp, dWr, s));    // R8 router
+  MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr, Xp, dz,
+                       dzp, at<float>(ws, W.dwr_part), dWr, s));                                      // R8 router
   prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
   if (shared) {

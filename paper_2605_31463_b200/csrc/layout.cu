@@ -92,6 +92,7 @@ WsLayout ws_layout(const moe_config_t* c) {
   L.dw = k.take(T * c->K * 4);
   L.dz = k.take(T * c->K * 4);
   L.dzp = k.take(R * 4);
+  L.dwr_part = k.take((R / 128 + 1) * H * 4);   // per-tile partial sums of dWr (fp32)
   L.dy = k.take(R * H * es);
   L.dgu = k.take(R * 2 * F * es);
   L.dXp = k.take(R * H * es);

@@ -1,6 +1,8 @@
 // Router: logits z = X Wr^T (R1), and the router backward dw -> dz -> dWr (R8).  SURVEY.md §8c.
 // dX += dz Wr is folded into the dX combine kernel (rows.cu).
-#include "common.cuh"
+#include <string.h>
+
+#include "gemm_tc.cuh"
 
 namespace moe {
 namespace {
@@ -119,9 +121,77 @@ __global__ void __launch_bounds__(256) dwr_kernel(const float* __restrict__ dzp,
   dWr[(size_t)e * H + h] = from_f<T>(acc);
 }
 
+
+// dWr on 128-row-aligned groups, in two deterministic passes that do not care how skewed the expert load is:
+//  pass 1: one CTA per (128-row tile, 256-column slab): part[tile, h] = sum over the tile's live rows of dzp[r] * Xp[r, h]
+//          (8 warps x 16 rows, 8 columns per lane with 16-byte loads, fixed-order shared-memory reduction);
+//  pass 2: dWr[e, h] = sum of the expert's tile partials in ascending tile order.
+__global__ void __launch_bounds__(256) dwr_tile_kernel(const float* __restrict__ dzp, const uint4* __restrict__ Xp,
+                                                       const int32_t* __restrict__ mtile,
+                                                       const int32_t* __restrict__ offsets,
+                                                       const int32_t* __restrict__ counts, int H,
+                                                       float* __restrict__ part) {
+  __shared__ float red[8][256];
+  const int tile = blockIdx.x;
+  if (tile >= mtile[0]) return;
+  const int e = mtile[1 + tile];
+  const int live_end = offsets[e] + counts[e];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int col = blockIdx.y * 256 + lane * 8;
+  float acc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i] = 0.f;
+  if (col < H) {
+    const int r0 = tile * 128 + warp * 16;
+#pragma unroll 4
+    for (int i = 0; i < 16; ++i) {
+      const int r = r0 + i;
+      if (r >= live_end) break;
+      const float d = dzp[r];
+      const uint4 v = __ldg(Xp + ((size_t)r * H + col) / 8);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        acc[2 * k] = fmaf(d, __uint_as_float(w[k] << 16), acc[2 * k]);
+        acc[2 * k + 1] = fmaf(d, __uint_as_float(w[k] & 0xffff0000u), acc[2 * k + 1]);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) red[warp][lane * 8 + i] = acc[i];
+  __syncthreads();
+  const int h = blockIdx.y * 256 + threadIdx.x;
+  if (h < H) {
+    float s = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
+    part[(size_t)tile * H + h] = s;
+  }
+}
+
+__global__ void __launch_bounds__(256) dwr_reduce_kernel(const float* __restrict__ part,
+                                                         const int32_t* __restrict__ offsets, int H,
+                                                         __nv_bfloat16* __restrict__ dWr) {
+  const int e = blockIdx.x;
+  const int h = blockIdx.y * 256 + threadIdx.x;
+  if (h >= H) return;
+  const int t0 = offsets[e] / 128, t1 = offsets[e + 1] / 128;
+  float s = 0.f;
+  for (int t = t0; t < t1; ++t) s += part[(size_t)t * H + h];
+  dWr[(size_t)e * H + h] = __float2bfloat16_rn(s);
+}
+
 }  // namespace
 
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s) {
+  if (c->dtype != 0 && c->H % 64 == 0 && c->E % 4 == 0) {   // bf16: tcgen05 GEMM with fp32 output (one group of T rows)
+    TcCall t;
+    memset(&t, 0, sizeof(t));
+    t.mode = TC_FWD_F32; t.E = 1; t.rows_cap = c->T; t.A = X; t.lda = c->H; t.B0 = Wr; t.b_rows = c->E; t.b_cols = c->H;
+    t.N = c->E; t.Kd = c->H; t.out0 = z; t.ld0 = c->E;
+    const int32_t st = tc_gemm(t, s);
+    if (st != MOE_ERR_UNSUPPORTED) return st;
+  }
   dim3 grid((unsigned)ceil_div(c->T, 64), (unsigned)ceil_div(c->E, 64));
   if (c->dtype == 0)
     MOE_LAUNCH(logits_kernel<float>, grid, 256, 0, s, (const float*)X, (const float*)Wr, c->T, c->H, c->E, z);
@@ -132,12 +202,17 @@ int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, floa
 }
 
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
-                   const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const void* Xp, float* dz,
-                   float* dzp, void* dWr, cudaStream_t s) {
+                   const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const int32_t* mtile,
+                   const void* Xp, float* dz, float* dzp, float* part, void* dWr, cudaStream_t s) {
   if (c->score_fn == 0 && !c->renorm) return MOE_ERR_UNSUPPORTED;  // dense dz: not on any config's path
   MOE_LAUNCH(dz_kernel, (unsigned)ceil_div(c->T, 4), 128, 0, s, z, idx, w, dw, f2p, c->T, c->E, c->K, c->score_fn,
              c->renorm, c->routed_scale, dz, dzp);
-  if (dWr) {
+  if (dWr && c->dtype != 0 && c->row_align % 128 == 0 && c->H % 8 == 0 && mtile && part) {
+    const unsigned slabs = (unsigned)ceil_div(c->H, 256);
+    MOE_LAUNCH(dwr_tile_kernel, dim3((unsigned)(padded_rows(c) / 128), slabs), 256, 0, s, dzp, (const uint4*)Xp, mtile,
+               offsets, counts, c->H, part);
+    MOE_LAUNCH(dwr_reduce_kernel, dim3((unsigned)c->E, slabs), 256, 0, s, part, offsets, c->H, (__nv_bfloat16*)dWr);
+  } else if (dWr) {
     dim3 grid((unsigned)c->E, (unsigned)ceil_div(c->H, 256));
     if (c->dtype == 0)
       MOE_LAUNCH(dwr_kernel<float>, grid, 256, 0, s, dzp, (const float*)Xp, offsets, counts, c->H, (float*)dWr);
