@@ -215,26 +215,48 @@ def run_cuda(args, cfg):
     for _ in range(max(3, args.warmup)):
         step()
     sync_all()
-    sampler = ClockSampler(local)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # ---- eager pass with the library's stage events on (stage table, launch count) ----
     moe.moe_profile_enable(True)
     n0 = moe.moe_launch_count()
-    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sync_all()
     ev0.record(stream)
     for _ in range(args.steps):
         step()
     ev1.record(stream)
     sync_all()
-    sampler.stop_flag = True
     launches = moe.moe_launch_count() - n0
-    ms = ev0.elapsed_time(ev1)
+    ms_eager = ev0.elapsed_time(ev1)
     stages = {}
     for name in moe.STAGES:
         t, n = moe.moe_profile_stage_ms(name)
         if n:
             stages[name] = {"ms_per_step": t / args.steps, "segments_per_step": n / args.steps}
     moe.moe_profile_enable(False)
+    # ---- timed region: the same step captured once into a CUDA graph (the library never synchronises or allocates,
+    # so fwd+bwd is capturable as is) and replayed K times; --no-graph times the eager launches instead ----
+    graph = None
+    if not args.no_graph:
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            lb.forward()
+            lb.backward()
+        for _ in range(3):
+            graph.replay()
+        sync_all()
+    sampler = ClockSampler(local)
+    sampler.start()
+    sync_all()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        if graph is not None:
+            graph.replay()
+        else:
+            step()
+    ev1.record(stream)
+    sync_all()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
     if world > 1:
         tmax = torch.tensor([ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -305,7 +327,8 @@ def run_cuda(args, cfg):
         cpu = {"value": f / t / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": desc,
                "seconds": t}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / args.steps, "ms_per_step_eager": ms_eager / args.steps,
+            "launch": "eager" if args.no_graph else "cuda_graph replay of fwd+bwd", "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.dtype], "data": "synthetic",
             "config": {"workload": cfg.name, "T": cfg.T, "H": cfg.H, "E": cfg.E, "K": cfg.K, "F": cfg.F,
                        "F_shared": cfg.F_shared, "row_align": cfg.row_align, "parallelism": f"replicas x{world}",
@@ -328,6 +351,7 @@ def main():
     ap.add_argument("--config", default="qwen3_30b_a3b_like")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="time eager launches instead of CUDA-graph replays")
     args = ap.parse_args()
     cfg = pick_config(args.config)
     if args.impl == "reference":

@@ -22,9 +22,11 @@ __device__ __forceinline__ void stg_stream(int4* p, const int4& v) {
 }
 
 // Xp[f2p[t*K+j]] = X[t] for j < K: token-major, the source row is read once and written K times.
-__global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __restrict__ X, int T, int K, int nvec,
+template <int KT>
+__global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __restrict__ X, int T, int Krt, int nvec,
                                                                  const int32_t* __restrict__ f2p,
                                                                  int4* __restrict__ Xp) {
+  const int K = KT > 0 ? KT : Krt;
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= T) return;
@@ -37,6 +39,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
       const int v = v0 + u * 32 + lane;
       if (v < nvec) buf[u] = ldg_stream(src + v);
     }
+#pragma unroll
     for (int j = 0; j < K; ++j) {
       int4* dst = Xp + (size_t)rows[j] * nvec;
 #pragma unroll
@@ -97,15 +100,16 @@ struct Vec<__nv_bfloat16> {
 };
 
 // Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
-template <typename T>
+template <typename T, int KT>
 __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
                                                                   const int32_t* __restrict__ f2p,
                                                                   const int4* __restrict__ add0,
                                                                   const float* __restrict__ dz,
                                                                   const int32_t* __restrict__ idx,
-                                                                  const int4* __restrict__ Wr, int Tn, int K, int nvec,
+                                                                  const int4* __restrict__ Wr, int Tn, int Krt, int nvec,
                                                                   int4* __restrict__ Y) {
   constexpr int N = Vec<T>::N;
+  const int K = KT > 0 ? KT : Krt;
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= Tn) return;
@@ -114,12 +118,26 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
     float acc[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) acc[i] = 0.f;
-    for (int j = 0; j < K; ++j) {
-      const float wj = w ? w[(size_t)t * K + j] : 1.0f;
-      float f[N];
-      Vec<T>::unpack(ldg_stream(y + (size_t)rows[j] * nvec + v), f);
+    if (KT > 0) {                       // all K row loads in flight before the first use
+      int4 q[KT > 0 ? KT : 1];
 #pragma unroll
-      for (int i = 0; i < N; ++i) acc[i] = fmaf(wj, f[i], acc[i]);
+      for (int j = 0; j < KT; ++j) q[j] = ldg_stream(y + (size_t)rows[j] * nvec + v);
+#pragma unroll
+      for (int j = 0; j < KT; ++j) {
+        const float wj = w ? w[(size_t)t * K + j] : 1.0f;
+        float f[N];
+        Vec<T>::unpack(q[j], f);
+#pragma unroll
+        for (int i = 0; i < N; ++i) acc[i] = fmaf(wj, f[i], acc[i]);
+      }
+    } else {
+      for (int j = 0; j < K; ++j) {
+        const float wj = w ? w[(size_t)t * K + j] : 1.0f;
+        float f[N];
+        Vec<T>::unpack(ldg_stream(y + (size_t)rows[j] * nvec + v), f);
+#pragma unroll
+        for (int i = 0; i < N; ++i) acc[i] = fmaf(wj, f[i], acc[i]);
+      }
     }
     if (add0) {
       float f[N];
@@ -141,35 +159,74 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
 }
 
 // dy[f2p[t*K+j]] = w[t,j] * dY[t];   dw[t,j] = <dY[t], y[f2p[t*K+j]]>.
-template <typename T>
+// One warp per token; per 16-byte column chunk the K rows of y are loaded together (KT > 0) and the K dot products are
+// kept in registers; lane partials are reduced by shuffles in a fixed order at the end.
+template <typename T, int KT>
 __global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4* __restrict__ dY,
                                                                       const int4* __restrict__ y,
                                                                       const float* __restrict__ w,
-                                                                      const int32_t* __restrict__ f2p, int Tn, int K,
+                                                                      const int32_t* __restrict__ f2p, int Tn, int Krt,
                                                                       int nvec, int4* __restrict__ dy,
                                                                       float* __restrict__ dw) {
   constexpr int N = Vec<T>::N;
+  const int K = KT > 0 ? KT : Krt;
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= Tn) return;
-  for (int j = 0; j < K; ++j) {
-    const int r = f2p[(size_t)t * K + j];
-    const float wj = w[(size_t)t * K + j];
-    float dot = 0.f;
-    for (int v = lane; v < nvec; v += 32) {
-      float g[N], f[N], o[N];
-      Vec<T>::unpack(__ldg(dY + (size_t)t * nvec + v), g);
-      Vec<T>::unpack(ldg_stream(y + (size_t)r * nvec + v), f);
+  if (KT > 0) {
+    int r[KT > 0 ? KT : 1];
+    float wj[KT > 0 ? KT : 1], dot[KT > 0 ? KT : 1];
 #pragma unroll
-      for (int i = 0; i < N; ++i) {
-        dot = fmaf(g[i], f[i], dot);
-        o[i] = wj * g[i];
+    for (int j = 0; j < KT; ++j) {
+      r[j] = f2p[(size_t)t * K + j];
+      wj[j] = w[(size_t)t * K + j];
+      dot[j] = 0.f;
+    }
+    for (int v = lane; v < nvec; v += 32) {
+      float g[N];
+      Vec<T>::unpack(ldg_stream(dY + (size_t)t * nvec + v), g);
+      int4 q[KT > 0 ? KT : 1];
+#pragma unroll
+      for (int j = 0; j < KT; ++j) q[j] = ldg_stream(y + (size_t)r[j] * nvec + v);
+#pragma unroll
+      for (int j = 0; j < KT; ++j) {
+        float f[N], o[N];
+        Vec<T>::unpack(q[j], f);
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          dot[j] = fmaf(g[i], f[i], dot[j]);
+          o[i] = wj[j] * g[i];
+        }
+        stg_stream(dy + (size_t)r[j] * nvec + v, Vec<T>::pack(o));
       }
-      stg_stream(dy + (size_t)r * nvec + v, Vec<T>::pack(o));
     }
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(FULL, dot, off);
-    if (lane == 0) dw[(size_t)t * K + j] = dot;
+    for (int j = 0; j < KT; ++j) {
+      float d = dot[j];
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) d += __shfl_xor_sync(FULL, d, off);
+      if (lane == 0) dw[(size_t)t * K + j] = d;
+    }
+  } else {
+    for (int j = 0; j < K; ++j) {
+      const int r = f2p[(size_t)t * K + j];
+      const float wj = w[(size_t)t * K + j];
+      float dot = 0.f;
+      for (int v = lane; v < nvec; v += 32) {
+        float g[N], f[N], o[N];
+        Vec<T>::unpack(__ldg(dY + (size_t)t * nvec + v), g);
+        Vec<T>::unpack(ldg_stream(y + (size_t)r * nvec + v), f);
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          dot = fmaf(g[i], f[i], dot);
+          o[i] = wj * g[i];
+        }
+        stg_stream(dy + (size_t)r * nvec + v, Vec<T>::pack(o));
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(FULL, dot, off);
+      if (lane == 0) dw[(size_t)t * K + j] = dot;
+    }
   }
 }
 
@@ -179,8 +236,16 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
                     const int32_t* offsets, void* Xp, cudaStream_t s) {
   if ((cols * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(cols * esz / 16);
-  MOE_LAUNCH(gather_kernel, (unsigned)ceil_div(c->T, ROW_WARPS), ROW_WARPS * 32, 0, s, (const int4*)X, c->T, c->K, nvec,
-             f2p, (int4*)Xp);
+#define MOE_GATHER(KT)                                                                                              \
+  MOE_LAUNCH(gather_kernel<KT>, (unsigned)ceil_div(c->T, ROW_WARPS), ROW_WARPS * 32, 0, s, (const int4*)X, c->T, c->K, \
+             nvec, f2p, (int4*)Xp)
+  switch (c->K) {
+    case 2: MOE_GATHER(2); break;
+    case 4: MOE_GATHER(4); break;
+    case 8: MOE_GATHER(8); break;
+    default: MOE_GATHER(0); break;
+  }
+#undef MOE_GATHER
   if (c->row_align > 1)
     MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)Xp);
   return MOE_OK;
@@ -192,12 +257,20 @@ int32_t combine(const moe_config_t* c, const void* y, const float* w, const int3
   if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(c->H * esz / 16);
   const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
-  if (c->dtype == 0)
-    MOE_LAUNCH(combine_kernel<float>, grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz, idx,
-               (const int4*)Wr, c->T, c->K, nvec, (int4*)Y);
-  else
-    MOE_LAUNCH(combine_kernel<__nv_bfloat16>, grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz,
-               idx, (const int4*)Wr, c->T, c->K, nvec, (int4*)Y);
+#define MOE_COMBINE(TY, KT)                                                                                       \
+  MOE_LAUNCH((combine_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz, idx, \
+             (const int4*)Wr, c->T, c->K, nvec, (int4*)Y)
+  if (c->dtype == 0) {
+    MOE_COMBINE(float, 0);
+  } else {
+    switch (c->K) {
+      case 2: MOE_COMBINE(__nv_bfloat16, 2); break;
+      case 4: MOE_COMBINE(__nv_bfloat16, 4); break;
+      case 8: MOE_COMBINE(__nv_bfloat16, 8); break;
+      default: MOE_COMBINE(__nv_bfloat16, 0); break;
+    }
+  }
+#undef MOE_COMBINE
   return MOE_OK;
 }
 
@@ -207,12 +280,20 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
   if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(c->H * esz / 16);
   const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
-  if (c->dtype == 0)
-    MOE_LAUNCH(combine_bwd_kernel<float>, grid, ROW_WARPS * 32, 0, s, (const int4*)dY, (const int4*)y, w, f2p, c->T,
-               c->K, nvec, (int4*)dy, dw);
-  else
-    MOE_LAUNCH(combine_bwd_kernel<__nv_bfloat16>, grid, ROW_WARPS * 32, 0, s, (const int4*)dY, (const int4*)y, w, f2p,
-               c->T, c->K, nvec, (int4*)dy, dw);
+#define MOE_COMBINE_BWD(TY, KT)                                                                                   \
+  MOE_LAUNCH((combine_bwd_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)dY, (const int4*)y, w, f2p, c->T, \
+             c->K, nvec, (int4*)dy, dw)
+  if (c->dtype == 0) {
+    MOE_COMBINE_BWD(float, 0);
+  } else {
+    switch (c->K) {
+      case 2: MOE_COMBINE_BWD(__nv_bfloat16, 2); break;
+      case 4: MOE_COMBINE_BWD(__nv_bfloat16, 4); break;
+      case 8: MOE_COMBINE_BWD(__nv_bfloat16, 8); break;
+      default: MOE_COMBINE_BWD(__nv_bfloat16, 0); break;
+    }
+  }
+#undef MOE_COMBINE_BWD
   if (c->row_align > 1)
     MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)dy);
   return MOE_OK;

@@ -71,3 +71,27 @@ def test_host_step_matches_device_step():
     lb.step_host(Xh, dYh, Yh, dXh)
     torch.cuda.synchronize()
     assert torch.equal(Yh, ref.Y.cpu()) and torch.equal(dXh, ref.dX.cpu())
+
+
+def test_cuda_graph_replay_matches_eager():
+    """The library neither synchronises nor allocates, so fwd+bwd can be captured into a CUDA graph (what bench.py
+    times); a replay on fresh inputs must reproduce the eager result bit for bit."""
+    import torch
+    cfg = wl.QWEN3_SMALL.replace(row_align=128)
+    inp = gc.gen_inputs(cfg)
+    ref = gc.run_gpu_layer(cfg, inp)
+    from paper_2605_31463_b200.buffers import LayerBuffers
+    lb = LayerBuffers(cfg)
+    lb.load(**inp)
+    lb.forward(); lb.backward()                      # warm-up: lazy function attributes are set outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        lb.forward()
+        lb.backward()
+    for t in (lb.Y, lb.dX, lb.dWg, lb.dWd, lb.dWr):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for name in ("Y", "dX", "dWr", "dWg", "dWu", "dWd"):
+        assert torch.equal(getattr(lb, name), getattr(ref, name)), name
