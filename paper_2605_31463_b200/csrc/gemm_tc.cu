@@ -11,6 +11,7 @@
 // Both K-major and MN-major shared-memory operand layouts are used, so the dgrad (weights read
 // "transposed") and wgrad (both operands contracted over rows) need no transposed copies in HBM.
 #include <cuda.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -67,8 +68,8 @@ bool tc_make_map3(CUtensorMap* m, const void* ptr, int64_t d0, int64_t d1, int64
   const cuuint32_t box[3] = {(cuuint32_t)box0, (cuuint32_t)box1, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            CU_TENSOR_MAP_INTERLEAVE_NONE, box0 == 32 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 int tc_sm_count() {
@@ -101,7 +102,7 @@ constexpr int TMEM_COLS = 512;
 // kernel parameters
 // ---------------------------------------------------------------------------------------------
 struct TcParams {
-  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0;
+  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, raster, tma_out;
   int64_t rows_valid;
   const int32_t* mtile;
   const int32_t* offsets;
@@ -133,11 +134,35 @@ __device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_
       tl.row0 = 0;
       tl.nkb = (int)((p.rows_valid + BK - 1) / BK);
     }
-  } else {
+  } else if (p.raster == 0) {
+    // n fastest: consecutive CTAs share the 128-row activation tile
     const int mt = (int)(t / p.n_tiles);
     tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
     tl.m0 = mt * BM;
     tl.e = p.mtile ? p.mtile[1 + mt] : 0;
+    tl.nkb = p.nkb;
+    tl.row0 = 0;
+  } else {
+    // expert major, then n, then m fastest: the CTAs that run side by side share the (twice larger) weight tile of
+    // one expert, so L2 serves it once to all of them
+    int e = 0, first = 0, m_cnt;
+    if (p.mtile) {
+      int lo = 0, hi = p.E;   // largest e with (offsets[e] / 128) * n_tiles <= t
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((int64_t)(__ldg(p.offsets + mid) >> 7) * p.n_tiles <= t) lo = mid; else hi = mid;
+      }
+      e = lo;
+      first = __ldg(p.offsets + e) >> 7;
+      m_cnt = (__ldg(p.offsets + e + 1) >> 7) - first;
+    } else {
+      m_cnt = (int)((p.rows_valid + BM - 1) / BM);
+    }
+    const int local = (int)(t - (int64_t)first * p.n_tiles);
+    const int nt = local / m_cnt;
+    tl.n0 = nt * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
+    tl.m0 = (first + local - nt * m_cnt) * BM;
+    tl.e = e;
     tl.nkb = p.nkb;
     tl.row0 = 0;
   }
@@ -255,13 +280,46 @@ __device__ __forceinline__ void gu_load(const TcParams& p, const Tile& tl, int64
     }
 }
 
+// Output path: with F % 32 == 0 the chunk's dg and du (32 columns x 128 rows each) are staged in the warp group's two
+// 64-byte-swizzled 8 KB boxes and written by TMA (full lines instead of 16-byte partial sectors per thread).
 __device__ __forceinline__ void dgrad_swiglu_chunk(const TcParams& p, const Tile& tl, int64_t row, bool row_ok, int c,
-                                                   uint32_t tacc, const GuChunk& k) {
+                                                   uint32_t tacc, const GuChunk& k, uint32_t obuf, int row_in_tile,
+                                                   const CUtensorMap* tmO, bool issuer, int ch) {
   const int ncols = p.F - (tl.n0 + c * 32);   // warp-uniform
   if (ncols <= 0) return;
   uint32_t d[32];
   tmem_ld32(tacc + c * 32, d);
   tmem_ld_wait();
+  if (p.tma_out) {
+    if (issuer) bulk_wait_read0();     // this group's previous stores have finished reading the boxes
+    named_bar_sync(1 + ch, 128);
+    const uint32_t rowaddr = obuf + row_in_tile * 64;
+    const int sw = (row_in_tile >> 1) & 3;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint32_t gw[4] = {k.g[q].x, k.g[q].y, k.g[q].z, k.g[q].w}, uw[4] = {k.u[q].x, k.u[q].y, k.u[q].z, k.u[q].w};
+      uint32_t og[4], ou[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+        const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
+        const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
+        og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
+        ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
+      }
+      if (!row_ok) og[0] = og[1] = og[2] = og[3] = ou[0] = ou[1] = ou[2] = ou[3] = 0u;   // clipped by the map anyway
+      st_shared_v4(rowaddr + ((q ^ sw) << 4), og[0], og[1], og[2], og[3]);
+      st_shared_v4(rowaddr + OBUF_BYTES / 2 + ((q ^ sw) << 4), ou[0], ou[1], ou[2], ou[3]);
+    }
+    fence_proxy_async();
+    named_bar_sync(1 + ch, 128);
+    if (issuer) {
+      tma_store_3d(tmO, obuf, tl.n0 + c * 32, tl.m0, 0);
+      tma_store_3d(tmO, obuf + OBUF_BYTES / 2, p.F + tl.n0 + c * 32, tl.m0, 0);
+      bulk_commit();
+    }
+    return;
+  }
   if (!row_ok) return;
   __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + tl.n0 + c * 32;
 #pragma unroll
@@ -290,7 +348,7 @@ __device__ __forceinline__ void dgrad_swiglu_chunk(const TcParams& p, const Tile
 // and alternate, so one group's TMA store overlaps the other group's TMEM drain.
 __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
                                                  bool have_acc, uint32_t obuf, const CUtensorMap* tmO, bool issuer,
-                                                 int ch) {
+                                                 int ch, int ecoord) {
 #pragma unroll 1
   for (int c = ch; c < BN / 64; c += 2) {
     const int ncols = p.N - (tl.n0 + c * 64);   // warp-uniform
@@ -322,7 +380,7 @@ __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& 
     fence_proxy_async();
     named_bar_sync(1 + ch, 128);
     if (issuer) {
-      tma_store_3d(tmO, obuf, tl.n0 + c * 64, tl.m0, tl.e);
+      tma_store_3d(tmO, obuf, tl.n0 + c * 64, tl.m0, ecoord);
       bulk_commit();
     }
   }
@@ -334,7 +392,7 @@ __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& 
 template <int MODE>
 __global__ void __launch_bounds__(NTHREADS, 1)
 tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
-               const __grid_constant__ CUtensorMap tmB1, const TcParams p) {
+               const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmO, const TcParams p) {
   constexpr bool A_MN = (MODE == TC_WGRAD);
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
   extern __shared__ uint8_t smem_raw[];
@@ -350,6 +408,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB0);
     tma_prefetch_desc(&tmB1);
+    tma_prefetch_desc(&tmO);
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full0 + 8 * s, 1);
       mbar_init(empty0 + 8 * s, 1);
@@ -451,6 +510,17 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       if (MODE == TC_DGRAD_SWIGLU) {
         const int64_t row = (int64_t)tl.m0 + row_in_tile;
         const bool row_ok = row < p.rows_valid;
+        {   // pull the NEXT tile's g, u rows into L2 a whole tile ahead (ch 0 warps take g, ch 1 warps take u)
+          Tile nx;
+          if (decode_tile<MODE>(p, t + gridDim.x, total, nx)) {
+            const int64_t nrow = (int64_t)nx.m0 + row_in_tile;
+            if (nrow < p.rows_valid) {
+              const __nv_bfloat16* src = p.gu + nrow * p.ldgu + (ch ? p.F : 0) + nx.n0;
+              const int ncol = min(BN, p.F - nx.n0);
+              for (int c = 0; c < ncol; c += 64) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + c));
+            }
+          }
+        }
         GuChunk k[3];
         gu_load(p, tl, row, row_ok, ch, k[0]);
         gu_load(p, tl, row, row_ok, ch + 2, k[1]);
@@ -459,14 +529,16 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
         for (int i = 0; i < BN / 64; ++i) {      // this warp's chunks: c = ch, ch + 2, ...
           if (i + 2 < BN / 64) gu_load(p, tl, row, row_ok, ch + 2 * (i + 2), k[(i + 2) % 3]);
-          dgrad_swiglu_chunk(p, tl, row, row_ok, ch + 2 * i, tacc, k[i % 3]);
+          dgrad_swiglu_chunk(p, tl, row, row_ok, ch + 2 * i, tacc, k[i % 3], obuf0 + ch * OBUF_BYTES, row_in_tile, &tmO,
+                             (threadIdx.x & 127) == 64, ch);
         }
-      } else if (MODE == TC_WGRAD) {
+      } else if (MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD) {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
           tc_fence_after();
         }
-        wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmB1, (threadIdx.x & 127) == 64, ch);
+        wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch,
+                         MODE == TC_WGRAD ? tl.e : 0);
       } else {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
@@ -481,7 +553,8 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
-    if (MODE == TC_WGRAD && (threadIdx.x & 127) == 64) bulk_wait0();   // all TMA stores complete before the CTA retires
+    if ((MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU) && (threadIdx.x & 127) == 64)
+      bulk_wait0();   // all TMA stores complete before the CTA retires
   }
   tc_fence_before();
   __syncthreads();
@@ -501,7 +574,8 @@ int g_sm_count = 0;
 bool g_attr_set[6] = {false, false, false, false, false, false};
 
 template <int MODE>
-int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const TcParams& p, int64_t max_tiles,
+int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
+               int64_t max_tiles,
                cudaStream_t s) {
   if (!g_attr_set[MODE]) {
     MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
@@ -513,7 +587,7 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
     MOE_CUDA(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
   }
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(g_sm_count, max_tiles));
-  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, p);
+  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, p);
   return MOE_OK;
 }
 
@@ -553,7 +627,15 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.M = c.M;
   p.b_rows = c.b_rows;
   p.a_col0 = c.a_col0;
-  CUtensorMap ta, tb0, tb1;
+  {
+    static int raster = -1;   // tile order of the row-grouped GEMMs: 0 = n fastest (default; measured 2% faster on configs[1]), MOE_TC_RASTER=1 = m fastest within an expert
+    if (raster < 0) {
+      const char* ev = getenv("MOE_TC_RASTER");
+      raster = ev ? atoi(ev) : 0;
+    }
+    p.raster = raster;
+  }
+  CUtensorMap ta, tb0, tb1, to;
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
   if (c.mode == TC_FWD_F32 ? ((c.N & 3) || (c.ld0 & 3)) : ((c.N & 7) || (c.ld0 & 7))) return MOE_ERR_UNSUPPORTED;
   switch (c.mode) {
@@ -564,8 +646,9 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       p.n_tiles = (int)ceil_div(c.N, BN);
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
-      if (c.mode == TC_FWD_F32) return launch<TC_FWD_F32>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
-      return launch<TC_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
+      if (c.mode == TC_FWD_F32) return launch<TC_FWD_F32>(ta, tb0, tb0, ta, p, max_mtiles * p.n_tiles, s);
+      if (!tc_make_map3(&to, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // C [rows, N]
+      return launch<TC_FWD>(ta, tb0, tb0, to, p, max_mtiles * p.n_tiles, s);
     }
     case TC_FWD_SWIGLU: {
       if (c.Kd % BK || (c.F & 7) || (c.ld1 & 7)) return MOE_ERR_UNSUPPORTED;
@@ -574,7 +657,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, c.B1, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
-      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, ta, p, max_mtiles * p.n_tiles, s);
     }
     case TC_DGRAD:
     case TC_DGRAD_SWIGLU: {
@@ -587,9 +670,14 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&ta, c.A, (int64_t)p.nkb * BK, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, split ? c.B1 : c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
-      if (c.mode == TC_DGRAD) return launch<TC_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      if (c.mode == TC_DGRAD) {
+        if (!tc_make_map3(&to, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dA [rows, N]
+        return launch<TC_DGRAD>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
+      }
       if ((c.F & 7) || (c.ldgu & 7)) return MOE_ERR_UNSUPPORTED;
-      return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // dg / du boxes of 32 columns must not straddle the [dg|du] boundary
+      if (!tc_make_map3(&to, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
+      return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
     }
     case TC_WGRAD: {
       p.m_tiles = (int)ceil_div(c.M, BM);
@@ -597,8 +685,8 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       // A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (inner = output columns)
       if (!make_map(&ta, c.A, c.lda, c.rows_cap, c.lda, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.A2, c.N, c.rows_cap, c.lda2, 64)) return MOE_ERR_UNSUPPORTED;
-      if (!tc_make_map3(&tb1, c.out0, c.N, c.M, c.E, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dB [E, M, N]
-      return launch<TC_WGRAD>(ta, tb0, tb1, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
+      if (!tc_make_map3(&to, c.out0, c.N, c.M, c.E, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dB [E, M, N]
+      return launch<TC_WGRAD>(ta, tb0, tb0, to, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
     }
   }
   return MOE_ERR_INVALID_ARG;
