@@ -522,14 +522,15 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           }
         }
         GuChunk k[3];
-        gu_load(p, tl, row, row_ok, ch, k[0]);
-        gu_load(p, tl, row, row_ok, ch + 2, k[1]);
+        constexpr int NC = BN / 64;              // chunks per warp: this warp drains columns [ch * 128, ch * 128 + 128)
+        gu_load(p, tl, row, row_ok, ch * NC, k[0]);
+        gu_load(p, tl, row, row_ok, ch * NC + 1, k[1]);
         mbar_wait(tfull0 + 8 * as, aphase);
         tc_fence_after();
 #pragma unroll
-        for (int i = 0; i < BN / 64; ++i) {      // this warp's chunks: c = ch, ch + 2, ...
-          if (i + 2 < BN / 64) gu_load(p, tl, row, row_ok, ch + 2 * (i + 2), k[(i + 2) % 3]);
-          dgrad_swiglu_chunk(p, tl, row, row_ok, ch + 2 * i, tacc, k[i % 3], obuf0 + ch * OBUF_BYTES, row_in_tile, &tmO,
+        for (int i = 0; i < NC; ++i) {
+          if (i + 2 < NC) gu_load(p, tl, row, row_ok, ch * NC + i + 2, k[(i + 2) % 3]);
+          dgrad_swiglu_chunk(p, tl, row, row_ok, ch * NC + i, tacc, k[i % 3], obuf0 + ch * OBUF_BYTES, row_in_tile, &tmO,
                              (threadIdx.x & 127) == 64, ch);
         }
       } else if (MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD) {
