@@ -32,11 +32,10 @@ __device__ __forceinline__ float block_scale(float amax, int mode) {
 }
 
 __device__ __forceinline__ uint32_t encode4(float a, float b, float c, float d, float scale) {
-  const uint32_t q0 = __nv_cvt_float_to_fp8(__fdiv_rn(a, scale), __NV_SATFINITE, __NV_E4M3);
-  const uint32_t q1 = __nv_cvt_float_to_fp8(__fdiv_rn(b, scale), __NV_SATFINITE, __NV_E4M3);
-  const uint32_t q2 = __nv_cvt_float_to_fp8(__fdiv_rn(c, scale), __NV_SATFINITE, __NV_E4M3);
-  const uint32_t q3 = __nv_cvt_float_to_fp8(__fdiv_rn(d, scale), __NV_SATFINITE, __NV_E4M3);
-  return q0 | (q1 << 8) | (q2 << 16) | (q3 << 24);
+  // cvt.rn.satfinite.e4m3x2.f32 packs two codes per instruction (.x -> low byte)
+  const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(a, scale), __fdiv_rn(b, scale)), __NV_SATFINITE, __NV_E4M3);
+  const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(c, scale), __fdiv_rn(d, scale)), __NV_SATFINITE, __NV_E4M3);
+  return lo | (hi << 16);
 }
 
 __device__ __forceinline__ void unpack8(const uint4& v, float (&f)[8]) {
@@ -82,50 +81,57 @@ __global__ void __launch_bounds__(256) quant_act_kernel(const uint4* __restrict_
   if (in_range && sub == 0) scales[blk] = s;
 }
 
-// 128x128 blocks over the last two axes: one CTA per block, 256 threads x 8 passes x 8 elements, kept in registers.
-__global__ void __launch_bounds__(256) quant_weight_kernel(const uint4* __restrict__ w, int rows, int cols, int rb,
-                                                           int cb, int mode, uint2* __restrict__ codes,
-                                                           float* __restrict__ scales) {
-  __shared__ float red[8];
+// 128x128 blocks over the last two axes: one CTA of 1024 threads per block, 2 passes x 8 elements per thread kept in
+// registers between the amax reduction and the encode (each element is read from HBM once); few registers per thread so
+// that two CTAs (64 warps) stay resident per SM and the load phase of one overlaps the encode phase of the other.
+constexpr int QW_THREADS = 1024;
+__global__ void __launch_bounds__(QW_THREADS, 2) quant_weight_kernel(const uint4* __restrict__ w, int rows, int cols,
+                                                                     int rb, int cb, int mode,
+                                                                     uint2* __restrict__ codes,
+                                                                     float* __restrict__ scales) {
+  __shared__ float red[QW_THREADS / 32];
   __shared__ float s_scale;
   const int bc = blockIdx.x % cb;
   const int br = (blockIdx.x / cb) % rb;
   const int64_t batch = blockIdx.x / (cb * rb);
-  const int sub = threadIdx.x & 15, r0 = threadIdx.x >> 4;   // 16 row-lanes per pass
+  const int sub = threadIdx.x & 15, r0 = threadIdx.x >> 4;   // 64 row-lanes per pass
   const int col = bc * 128 + sub * 8;
-  float f[8][8];
+  uint4 raw[2];
   float m = 0.f;
 #pragma unroll
-  for (int p = 0; p < 8; ++p) {
-    const int row = br * 128 + p * 16 + r0;
-    if (row < rows && col < cols) {
-      unpack8(w[((batch * rows + row) * cols + col) >> 3], f[p]);
-    } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) f[p][i] = 0.f;
-    }
-    m = fmaxf(m, amax8(f[p]));
+  for (int p = 0; p < 2; ++p) {
+    const int row = br * 128 + p * 64 + r0;
+    raw[p] = make_uint4(0u, 0u, 0u, 0u);
+    if (row < rows && col < cols) raw[p] = __ldg(w + (((batch * rows + row) * cols + col) >> 3));
+    float f[8];
+    unpack8(raw[p], f);
+    m = fmaxf(m, amax8(f));
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, off));
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
   __syncthreads();
-  if (threadIdx.x == 0) {
-    float mm = red[0];
+  if (threadIdx.x < 32) {
+    float mm = red[threadIdx.x];
 #pragma unroll
-    for (int i = 1; i < 8; ++i) mm = fmaxf(mm, red[i]);
-    const float s = block_scale(mm, mode);
-    s_scale = s;
-    scales[blockIdx.x] = s;              // [batch, rb, cb] == blockIdx order
+    for (int off = 16; off > 0; off >>= 1) mm = fmaxf(mm, __shfl_xor_sync(FULL, mm, off));
+    if (threadIdx.x == 0) {
+      const float s = block_scale(mm, mode);
+      s_scale = s;
+      scales[blockIdx.x] = s;            // [batch, rb, cb] == blockIdx order
+    }
   }
   __syncthreads();
   const float s = s_scale;
 #pragma unroll
-  for (int p = 0; p < 8; ++p) {
-    const int row = br * 128 + p * 16 + r0;
-    if (row < rows && col < cols)
+  for (int p = 0; p < 2; ++p) {
+    const int row = br * 128 + p * 64 + r0;
+    if (row < rows && col < cols) {
+      float f[8];
+      unpack8(raw[p], f);
       codes[((batch * rows + row) * cols + col) >> 3] =
-          make_uint2(encode4(f[p][0], f[p][1], f[p][2], f[p][3], s), encode4(f[p][4], f[p][5], f[p][6], f[p][7], s));
+          make_uint2(encode4(f[0], f[1], f[2], f[3], s), encode4(f[4], f[5], f[6], f[7], s));
+    }
   }
 }
 
@@ -161,7 +167,7 @@ int32_t fp8_quantize_weight(const void* w, int batch, int rows, int cols, int mo
   const int rb = (rows + 127) / 128, cb = (cols + 127) / 128;
   const int64_t blocks = (int64_t)batch * rb * cb;
   if (blocks >= (1ll << 31)) return MOE_ERR_UNSUPPORTED;
-  MOE_LAUNCH(quant_weight_kernel, (unsigned)blocks, 256, 0, s, (const uint4*)w, rows, cols, rb, cb, mode, (uint2*)codes,
+  MOE_LAUNCH(quant_weight_kernel, (unsigned)blocks, QW_THREADS, 0, s, (const uint4*)w, rows, cols, rb, cb, mode, (uint2*)codes,
              scales);
   return MOE_OK;
 }
