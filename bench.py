@@ -28,6 +28,11 @@ import workloads as wl  # noqa: E402
 METRIC = "moe_layer_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 NOMINAL = {"bf16_tflops": 2250.0, "hbm_gbs": 8000.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each GEMM stage's kernel, from the `ncu --set full` capture
+# summarised in profiles/r1c_step_full.md (configs[1] only; other workloads report traffic = null).
+NCU_TRAFFIC = {"qwen3_30b_a3b_like": {"gemm1_swiglu": 1.112e9 + 314.4e6, "gemm2": 0.517e9 + 272.1e6,
+                                      "dgrad_down_swiglu": 1.171e9 + 198.9e6, "dgrad_gateup": 1.034e9 + 287.2e6,
+                                      "wgrad": 0.419e9 + 360.4e6}}
 
 
 def load_peaks():
@@ -308,10 +313,13 @@ def run_cuda(args, cfg):
         st = stages[dom]
         nl = 3 if dom == "wgrad" else 1
         tc = "tflops" in st and cfg.dtype != wl.DTYPE_FP32
+        fp8_stage = cfg.dtype == wl.DTYPE_FP8 and dom != "wgrad"     # fprop and dgrad run on e4m3 codes, wgrad on bf16
+        peak = peaks["bf16_sustained"] * (2.0 if fp8_stage else 1.0)  # fp8 peak = measured bf16 x the nominal 2:1 ratio
         roofline = {"bound": "tensor" if tc else "alu", "kernel": dom, "achieved": st.get("tflops"),
-                    "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
-                    "frac": (st["tflops"] / peaks["bf16_sustained"]) if "tflops" in st else None,
-                    "traffic": None, "launches_per_step": nl, "ms_per_launch": st["ms_per_step"] / nl,
+                    "peak": peak, "unit": "TFLOP/s",
+                    "frac": (st["tflops"] / peak) if "tflops" in st else None,
+                    "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(dom), "traffic_unit": "bytes per launch (ncu dram read+write)",
+                    "algorithmic_flops_per_launch": sf[dom] / nl, "launches_per_step": nl, "ms_per_launch": st["ms_per_step"] / nl,
                     "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
                     "frac_nominal_2250": st.get("frac_nominal")}
     rp = [stages[n]["ms_per_step"] for n in ("route", "maps", "permute") if n in stages]

@@ -51,18 +51,15 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
   }
 }
 
-// Zero the padding rows (perm_to_flat[r] < 0) below offsets[E].
+// Zero the padding rows (perm_to_flat[r] < 0) below offsets[E]: one warp per row, every row's map entry read in parallel.
 __global__ void __launch_bounds__(ROW_WARPS * 32) zero_pad_kernel(const int32_t* __restrict__ p2f,
                                                                    const int32_t* __restrict__ offsets, int E,
-                                                                   int nvec, int4* __restrict__ Xp) {
+                                                                   int nvec, int64_t rows_cap, int4* __restrict__ Xp) {
   const int lane = threadIdx.x & 31;
-  const int rows = offsets[E];
-  const int wstride = gridDim.x * ROW_WARPS;
-  for (int r = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5); r < rows; r += wstride) {
-    if (p2f[r] >= 0) continue;
-    int4* dst = Xp + (size_t)r * nvec;
-    for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
-  }
+  const int64_t r = (int64_t)blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
+  if (r >= rows_cap || r >= offsets[E] || p2f[r] >= 0) return;
+  int4* dst = Xp + (size_t)r * nvec;
+  for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
 }
 
 template <typename T>
@@ -247,7 +244,8 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
   }
 #undef MOE_GATHER
   if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)Xp);
+    MOE_LAUNCH(zero_pad_kernel, (unsigned)ceil_div(padded_rows(c), ROW_WARPS), ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec,
+               padded_rows(c), (int4*)Xp);
   return MOE_OK;
 }
 
@@ -295,7 +293,8 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
   }
 #undef MOE_COMBINE_BWD
   if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, 148 * 4, ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec, (int4*)dy);
+    MOE_LAUNCH(zero_pad_kernel, (unsigned)ceil_div(padded_rows(c), ROW_WARPS), ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec,
+               padded_rows(c), (int4*)dy);
   return MOE_OK;
 }
 
