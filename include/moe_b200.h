@@ -158,6 +158,17 @@ int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const void* X, co
                       const void* ctx, void* dX, void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s,
                       void* dWu_s, void* dWd_s, void* ws, void* stream);
 
+/* R8, weight gradients only -- the separately schedulable half of the backward that a delayed weight-gradient
+ * schedule needs (PAPER.md:116 "wgrad delay", :239).  Call moe_layer_bwd with NULL weight gradients first (dgrad, dX,
+ * dWr), then this at any later point of the same stream order; `ctx` and `ws` must be the untouched buffers of those
+ * calls (it reads Xp, a from ctx and dy, dgu from ws).  X, dY are the layer input and output gradient (used by the
+ * shared expert).  accumulate_fp32 = 0: gradients in the weights' type, overwritten (as moe_layer_bwd);
+ * accumulate_fp32 = 1: dW* are fp32 tensors of the weights' shapes and the new gradient is ADDED to them (fp32 main
+ * gradients across micro-batches); tensor-core path only (dtype 1 or 2, row_align % 128 == 0), else UNSUPPORTED. */
+int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const void* dY, const void* ctx, const void* ws,
+                        void* dWg, void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s,
+                        int32_t accumulate_fp32, void* stream);
+
 /* End-to-end step with HOST activations: copies X_host and dY_host [T,H] to the device buffers
  * X_dev / dY_dev, runs moe_layer_fwd + moe_layer_bwd, copies Y and dX back to Y_host / dX_host, all on
  * `stream` (host buffers should be pinned; returns without synchronising).  Weights, gradients, ctx,

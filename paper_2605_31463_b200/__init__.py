@@ -62,6 +62,7 @@ _SIGNATURES = {
     "moe_fp8_quantize_weights": (_I32, [_CFG] + [_P] * 8),
     "moe_layer_fwd": (_I32, [_CFG] + [_P] * 15),
     "moe_layer_bwd": (_I32, [_CFG] + [_P] * 20),
+    "moe_layer_wgrad": (_I32, [_CFG] + [_P] * 10 + [_I32, _P]),
     "moe_layer_step_host": (_I32, [_CFG] + [_P] * 28),
     "moe_ctx_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
     "moe_ws_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
@@ -232,6 +233,12 @@ def moe_layer_bwd(cfg, dY, X, Wr, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, dX, dWr, dW
                                _ptr(Wg_s), _ptr(Wu_s), _ptr(Wd_s), _ptr(ctx), _ptr(dX), _ptr(dWr), _ptr(dWg),
                                _ptr(dWu), _ptr(dWd), _ptr(dWg_s), _ptr(dWu_s), _ptr(dWd_s), _ptr(ws),
                                _stream(stream)), "moe_layer_bwd")
+
+
+def moe_layer_wgrad(cfg, X, dY, ctx, ws, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, accumulate_fp32, stream=None):
+    _check(lib().moe_layer_wgrad(C.byref(make_config(cfg)), _ptr(X), _ptr(dY), _ptr(ctx), _ptr(ws), _ptr(dWg), _ptr(dWu),
+                                 _ptr(dWd), _ptr(dWg_s), _ptr(dWu_s), _ptr(dWd_s), int(accumulate_fp32), _stream(stream)),
+           "moe_layer_wgrad")
 
 
 def moe_layer_step_host(cfg, X_host, dY_host, Y_host, dX_host, X_dev, dY_dev, Y_dev, dX_dev, Wr, bias, Wg, Wu, Wd,

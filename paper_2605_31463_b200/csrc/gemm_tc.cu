@@ -59,16 +59,18 @@ bool tc_make_map(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t inner,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-bool tc_make_map3(CUtensorMap* m, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0, int box1) {
+bool tc_make_map3(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0,
+                  int box1) {
   EncodeTiledFn fn = encode_fn();
   if (!fn || !ptr || d0 <= 0 || d1 <= 0 || d2 <= 0) return false;
-  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || ((ld * 2) & 15)) return false;
+  if ((reinterpret_cast<uintptr_t>(ptr) & 15) || ((ld * elem_bytes) & 15)) return false;
   const cuuint64_t dims[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
-  const cuuint64_t strides[2] = {(cuuint64_t)ld * 2, (cuuint64_t)d1 * ld * 2};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * elem_bytes, (cuuint64_t)d1 * ld * elem_bytes};
   const cuuint32_t box[3] = {(cuuint32_t)box0, (cuuint32_t)box1, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
-  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, box0 == 32 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+  return fn(m, elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3,
+            const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            box0 * elem_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -102,7 +104,7 @@ constexpr int TMEM_COLS = 512;
 // kernel parameters
 // ---------------------------------------------------------------------------------------------
 struct TcParams {
-  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, raster, tma_out;
+  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, raster, tma_out, acc_f32;
   int64_t rows_valid;
   const int32_t* mtile;
   const int32_t* offsets;
@@ -386,6 +388,33 @@ __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& 
   }
 }
 
+// TC_WGRAD with fp32 accumulation into an existing gradient (dB += tile; PAPER.md:116 wgrad delay keeps fp32 main
+// gradients across micro-batches): 32-column fp32 chunks (128-byte rows) staged like above and added by a TMA
+// reduce-add store, so the old gradient is never read by the SM.  An empty expert adds nothing.
+__device__ __forceinline__ void wgrad_accum_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
+                                                 uint32_t obuf, const CUtensorMap* tmO, bool issuer, int ch) {
+#pragma unroll 1
+  for (int c = ch; c < BN / 32; c += 2) {
+    const int ncols = p.N - (tl.n0 + c * 32);   // warp-uniform
+    if (ncols <= 0) break;
+    uint32_t v[32];
+    tmem_ld32(tacc + c * 32, v);
+    tmem_ld_wait();
+    if (issuer) bulk_wait_read0();
+    named_bar_sync(1 + ch, 128);
+    const uint32_t rowaddr = obuf + row_in_tile * 128;
+    const int sw = row_in_tile & 7;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) st_shared_v4(rowaddr + ((j ^ sw) << 4), v[j * 4], v[j * 4 + 1], v[j * 4 + 2], v[j * 4 + 3]);
+    fence_proxy_async();
+    named_bar_sync(1 + ch, 128);
+    if (issuer) {
+      tma_reduce_add_3d(tmO, obuf, tl.n0 + c * 32, tl.m0, tl.e);
+      bulk_commit();
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
@@ -538,8 +567,12 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           mbar_wait(tfull0 + 8 * as, aphase);
           tc_fence_after();
         }
-        wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch,
-                         MODE == TC_WGRAD ? tl.e : 0);
+        if (MODE == TC_WGRAD && p.acc_f32) {
+          if (have) wgrad_accum_tile(p, tl, tacc, row_in_tile, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch);
+        } else {
+          wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch,
+                           MODE == TC_WGRAD ? tl.e : 0);
+        }
       } else {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
@@ -648,7 +681,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
       if (c.mode == TC_FWD_F32) return launch<TC_FWD_F32>(ta, tb0, tb0, ta, p, max_mtiles * p.n_tiles, s);
-      if (!tc_make_map3(&to, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // C [rows, N]
+      if (!tc_make_map3(&to, 2, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // C [rows, N]
       return launch<TC_FWD>(ta, tb0, tb0, to, p, max_mtiles * p.n_tiles, s);
     }
     case TC_FWD_SWIGLU: {
@@ -672,12 +705,12 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, split ? c.B1 : c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (c.mode == TC_DGRAD) {
-        if (!tc_make_map3(&to, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dA [rows, N]
+        if (!tc_make_map3(&to, 2, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dA [rows, N]
         return launch<TC_DGRAD>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
       }
       if ((c.F & 7) || (c.ldgu & 7)) return MOE_ERR_UNSUPPORTED;
       p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // dg / du boxes of 32 columns must not straddle the [dg|du] boundary
-      if (!tc_make_map3(&to, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
+      if (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
       return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
     }
     case TC_WGRAD: {
@@ -686,7 +719,10 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       // A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (inner = output columns)
       if (!make_map(&ta, c.A, c.lda, c.rows_cap, c.lda, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.A2, c.N, c.rows_cap, c.lda2, 64)) return MOE_ERR_UNSUPPORTED;
-      if (!tc_make_map3(&to, c.out0, c.N, c.M, c.E, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dB [E, M, N]
+      p.acc_f32 = c.acc_f32 ? 1 : 0;
+      if (c.acc_f32 ? !tc_make_map3(&to, 4, c.out0, c.N, c.M, c.E, c.ld0, 32, BM)    // fp32 dB [E, M, N], reduce-add
+                    : !tc_make_map3(&to, 2, c.out0, c.N, c.M, c.E, c.ld0, 64, BM))   // bf16 dB [E, M, N], overwrite
+        return MOE_ERR_UNSUPPORTED;
       return launch<TC_WGRAD>(ta, tb0, tb0, to, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
     }
   }

@@ -36,6 +36,7 @@ struct TcCall {
   void* out1; int ld1;       // FWD_SWIGLU: a
   const void* gu; int ldgu;  // DGRAD_SWIGLU: saved [g|u]
   int F;                     // SwiGLU width
+  int acc_f32;               // WGRAD: out0 is fp32 [E,M,N] and the tile is ADDED to it (ld0 in fp32 elements)
 };
 
 // Returns MOE_ERR_UNSUPPORTED (nothing enqueued) if the shape does not fit the tensor-core path.

@@ -69,6 +69,36 @@ int32_t ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* W
   return MOE_OK;
 }
 
+// The three weight gradients of one FFN group from the bf16 tensors (R8; R9: wgrad stays in bf16):
+//   dWd[e] = dy_e^T a_e,  dWg[e] = dg_e^T Xp_e,  dWu[e] = du_e^T Xp_e.
+// acc_f32: the outputs are fp32 buffers that the tiles are ADDED to (tensor-core path only).
+int32_t ffn_wgrad(const FfnGroup& g, const void* dy, const void* Xp, const void* a, const void* dgu, void* dWg, void* dWu,
+                  void* dWd, int acc_f32, cudaStream_t s) {
+  const bool tc_ok = g.dtype != 0 && g.H % 64 == 0 && g.F % 64 == 0 && (g.mtile != nullptr || g.E == 1);
+  if (tc_ok) {
+    TcCall c = tc_base(g, TC_WGRAD);
+    c.acc_f32 = acc_f32;
+    c.A = dy; c.lda = g.H; c.M = g.H; c.A2 = a; c.lda2 = g.F; c.N = g.F; c.out0 = dWd; c.ld0 = g.F;
+    MOE_CHECK(tc_gemm(c, s));
+    c = tc_base(g, TC_WGRAD);
+    c.acc_f32 = acc_f32;
+    c.A = dgu; c.lda = 2 * g.F; c.M = g.F; c.A2 = Xp; c.lda2 = g.H; c.N = g.H; c.out0 = dWg; c.ld0 = g.H;
+    MOE_CHECK(tc_gemm(c, s));
+    c.a_col0 = g.F; c.out0 = dWu;
+    MOE_CHECK(tc_gemm(c, s));
+    prof_mark(g.st_wgrad, s);
+    return MOE_OK;
+  }
+  if (acc_f32 || g.dtype == 2) return MOE_ERR_UNSUPPORTED;
+  const size_t es = g.dtype == 0 ? 4 : 2;
+  const void* dgu_u = (const char*)dgu + g.F * es;
+  MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.H, g.F, a, g.F, nullptr, dy, g.H, g.offsets, dWd, 0, g.rows_cap, 0, s));
+  MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu, 2 * g.F, g.offsets, dWg, 0, g.rows_cap, 0, s));
+  MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu_u, 2 * g.F, g.offsets, dWu, 0, g.rows_cap, 0, s));
+  prof_mark(g.st_wgrad, s);
+  return MOE_OK;
+}
+
 // dy [rows,H] -> dgu, dXp and (optionally) dWg, dWu, dWd.  da_tmp [rows,F] is scratch (CUDA-core path only).
 int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* gu, const void* a, const void* Wg,
                 const void* Wu, const void* Wd, void* da_tmp, void* dgu, void* dXp, void* dWg, void* dWu, void* dWd,
@@ -85,17 +115,7 @@ int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* g
     c.A = dgu; c.lda = 2 * g.F; c.B0 = Wg; c.B1 = Wu; c.b_rows = g.F; c.b_cols = g.H; c.N = g.H; c.out0 = dXp; c.ld0 = g.H;
     MOE_CHECK(tc_gemm(c, s));
     prof_mark(g.st_bwd2, s);
-    if (dWd) {
-      c = tc_base(g, TC_WGRAD);               // dWd[e] = dy_e^T a_e
-      c.A = dy; c.lda = g.H; c.M = g.H; c.A2 = a; c.lda2 = g.F; c.N = g.F; c.out0 = dWd; c.ld0 = g.F;
-      MOE_CHECK(tc_gemm(c, s));
-      c = tc_base(g, TC_WGRAD);               // dWg[e] = dg_e^T Xp_e, dWu[e] = du_e^T Xp_e
-      c.A = dgu; c.lda = 2 * g.F; c.M = g.F; c.A2 = Xp; c.lda2 = g.H; c.N = g.H; c.out0 = dWg; c.ld0 = g.H;
-      MOE_CHECK(tc_gemm(c, s));
-      c.a_col0 = g.F; c.out0 = dWu;
-      MOE_CHECK(tc_gemm(c, s));
-      prof_mark(g.st_wgrad, s);
-    }
+    if (dWd) MOE_CHECK(ffn_wgrad(g, dy, Xp, a, dgu, dWg, dWu, dWd, 0, s));
     return MOE_OK;
   }
   // da = dy Wd[e]            (B = Wd [E,H,F]: N = H, Kdim = F)
@@ -106,12 +126,7 @@ int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* g
   MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wg, dgu, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 0, s));
   MOE_CHECK(simt_grouped_gemm(1, g.dtype, g.E, g.F, g.H, nullptr, 0, Wu, dgu_u, 2 * g.F, g.offsets, dXp, g.H, g.rows_cap, 1, s));
   prof_mark(g.st_bwd2, s);
-  if (dWd) {
-    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.H, g.F, a, g.F, nullptr, dy, g.H, g.offsets, dWd, 0, g.rows_cap, 0, s));
-    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu, 2 * g.F, g.offsets, dWg, 0, g.rows_cap, 0, s));
-    MOE_CHECK(simt_grouped_gemm(2, g.dtype, g.E, g.F, g.H, Xp, g.H, nullptr, dgu_u, 2 * g.F, g.offsets, dWu, 0, g.rows_cap, 0, s));
-    prof_mark(g.st_wgrad, s);
-  }
+  if (dWd) MOE_CHECK(ffn_wgrad(g, dy, Xp, a, dgu, dWg, dWu, dWd, 0, s));
   return MOE_OK;
 }
 
@@ -169,18 +184,7 @@ int32_t ffn_bwd_fp8(const FfnGroup& g, const Fp8Bufs& q, const void* dy, const v
   c.b1_scales = q.Wuq_s; c.b_rows = g.F; c.b_cols = g.H; c.N = g.H; c.out0 = dXp; c.ld0 = g.H;
   MOE_CHECK(fp8_gemm(c, s));
   prof_mark(g.st_bwd2, s);
-  if (dWd) {
-    if (!(g.mtile != nullptr || g.E == 1)) return MOE_ERR_UNSUPPORTED;
-    TcCall t = tc_base(g, TC_WGRAD);
-    t.A = dy; t.lda = g.H; t.M = g.H; t.A2 = a; t.lda2 = g.F; t.N = g.F; t.out0 = dWd; t.ld0 = g.F;
-    MOE_CHECK(tc_gemm(t, s));
-    t = tc_base(g, TC_WGRAD);
-    t.A = dgu; t.lda = 2 * g.F; t.M = g.F; t.A2 = Xp; t.lda2 = g.H; t.N = g.H; t.out0 = dWg; t.ld0 = g.H;
-    MOE_CHECK(tc_gemm(t, s));
-    t.a_col0 = g.F; t.out0 = dWu;
-    MOE_CHECK(tc_gemm(t, s));
-    prof_mark(g.st_wgrad, s);
-  }
+  if (dWd) MOE_CHECK(ffn_wgrad(g, dy, Xp, a, dgu, dWg, dWu, dWd, 0, s));
   return MOE_OK;
 }
 
@@ -395,5 +399,34 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]
   MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, dz, idx, Wr, dX, s));
   prof_mark(ST_DX_COMBINE, s);
+  return MOE_OK;
+}
+
+// The weight-gradient half of the backward on its own (the layer-level piece of a delayed wgrad):
+// reads what moe_layer_fwd left in ctx (Xp, a) and what a preceding moe_layer_bwd (called with NULL weight gradients)
+// left in ws (dy, dgu), which therefore must not be reused in between.
+extern "C" int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const void* dY, const void* ctx, const void* ws,
+                                   void* dWg, void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s,
+                                   int32_t accumulate_fp32, void* stream) {
+  if (!cfg || !X || !dY || !ctx || !ws || !dWg || !dWu || !dWd) return MOE_ERR_INVALID_ARG;
+  MOE_CHECK(validate(cfg));
+  const bool shared = cfg->F_shared > 0;
+  const bool wgrad_s = dWg_s || dWu_s || dWd_s;
+  if (wgrad_s && !(shared && dWg_s && dWu_s && dWd_s)) return MOE_ERR_INVALID_ARG;
+  cudaStream_t s = as_stream(stream);
+  const CtxLayout C = ctx_layout(cfg);
+  const WsLayout W = ws_layout(cfg);
+  const int32_t* offsets = at<int32_t>(ctx, C.offsets);
+  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, at<int32_t>(ctx, C.counts),
+             (cfg->row_align % 128 == 0) ? at<int32_t>(ctx, C.mtile) : nullptr, cfg->row_align,
+             ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  prof_mark(ST_BEGIN, s);
+  MOE_CHECK(ffn_wgrad(g, at<char>(ws, W.dy), at<char>(ctx, C.Xp), at<char>(ctx, C.a), at<char>(ws, W.dgu), dWg, dWu, dWd,
+                      accumulate_fp32 ? 1 : 0, s));
+  if (wgrad_s) {
+    FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, offsets + cfg->E + 1, nullptr, nullptr, 1,
+                ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
+    MOE_CHECK(ffn_wgrad(gs, dY, X, at<char>(ctx, C.a_s), at<char>(ws, W.dgu_s), dWg_s, dWu_s, dWd_s, accumulate_fp32 ? 1 : 0, s));
+  }
   return MOE_OK;
 }

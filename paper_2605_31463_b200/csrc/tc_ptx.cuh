@@ -50,6 +50,12 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, uint32_t sr
                "r"(c0), "r"(c1), "r"(c2)
                : "memory");
 }
+// shared -> global tile reduction: global += shared (element type and box from the tensor map)
+__device__ __forceinline__ void tma_reduce_add_3d(const CUtensorMap* map, uint32_t src, int c0, int c1, int c2) {
+  asm volatile("cp.reduce.async.bulk.tensor.3d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
+               "r"(src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -133,8 +139,10 @@ __device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w 
 // zero fill out of bounds (gemm_tc.cu).
 bool tc_make_map(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t inner, int64_t outer, int64_t ld,
                  int box_inner, int box_outer);
-// 3-D bf16 map over [d2, d1, d0] (d0 contiguous, row pitch ld elements, d2 pitch d1 * ld), box = 1 x box1 x box0.
-bool tc_make_map3(CUtensorMap* m, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0, int box1);
+// 3-D map over [d2, d1, d0] elements of 2 (bf16) or 4 (fp32) bytes (d0 contiguous, row pitch ld elements, d2 pitch
+// d1 * ld), box = 1 x box1 x box0; 64-byte swizzle when a box row is 64 bytes, else 128-byte swizzle.
+bool tc_make_map3(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0,
+                  int box1);
 int tc_sm_count();
 
 }  // namespace moe

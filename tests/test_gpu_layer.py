@@ -95,3 +95,50 @@ def test_cuda_graph_replay_matches_eager():
     torch.cuda.synchronize()
     for name in ("Y", "dX", "dWr", "dWg", "dWu", "dWd"):
         assert torch.equal(getattr(lb, name), getattr(ref, name)), name
+
+
+WGRAD_CASES = [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128),
+               wl.DSV3_SMALL.replace(name="dsv3_small_align128", row_align=128),
+               wl.GPTOSS_SMALL.replace(name="gptoss_small_align128", row_align=128),
+               wl.DSV3_FP8_SMALL.replace(name="dsv3_fp8_small_align128", row_align=128)]
+
+
+@pytest.mark.parametrize("cfg", WGRAD_CASES, ids=lambda c: c.name)
+def test_delayed_wgrad_overwrite_and_fp32_accumulate(cfg):
+    """moe_layer_wgrad after a dgrad-only backward (PAPER.md:116 wgrad delay): (a) bf16 overwrite reproduces the fused
+    backward bit for bit; (b) fp32 accumulation adds the gradient to what the buffers held (two calls add it twice;
+    an empty expert's slice is untouched)."""
+    import torch
+    import paper_2605_31463_b200 as moe
+    from paper_2605_31463_b200.buffers import LayerBuffers, to_numpy
+    inp = gc.gen_inputs(cfg)
+    full = gc.run_gpu_layer(cfg, inp)
+    lb = LayerBuffers(cfg, with_grads=False)
+    lb.load(**inp)
+    lb.forward(); lb.backward()
+    names = ["dWg", "dWu", "dWd"] + (["dWg_s", "dWu_s", "dWd_s"] if cfg.F_shared else [])
+    out = {n: torch.full_like(getattr(full, n), 7.0) for n in names}
+    args = [out.get(n) for n in ("dWg", "dWu", "dWd", "dWg_s", "dWu_s", "dWd_s")]
+    moe.moe_layer_wgrad(lb.ccfg, lb.X, lb.dY, lb.ctx, lb.ws, *args, 0)
+    torch.cuda.synchronize()
+    assert torch.equal(lb.dX, full.dX)
+    for n in names:
+        assert torch.equal(out[n], getattr(full, n)), n
+    g0 = {n: torch.randn(getattr(full, n).shape, device="cuda", dtype=torch.float32) for n in names}
+    acc = {n: g0[n].clone() for n in names}
+    args = [acc.get(n) for n in ("dWg", "dWu", "dWd", "dWg_s", "dWu_s", "dWd_s")]
+    moe.moe_layer_wgrad(lb.ccfg, lb.X, lb.dY, lb.ctx, lb.ws, *args, 1)
+    moe.moe_layer_wgrad(lb.ccfg, lb.X, lb.dY, lb.ctx, lb.ws, *args, 1)
+    torch.cuda.synchronize()
+    counts = to_numpy(lb.ctx_view("counts"))
+    for n in names:
+        added = (acc[n] - g0[n]).double().cpu().numpy()
+        ref = 2.0 * to_numpy(getattr(full, n)).astype(np.float64)          # the bf16 gradient, itself oracle-checked
+        if added.ndim == 3:
+            for e in range(cfg.E):
+                if counts[e] == 0:
+                    assert torch.equal(acc[n][e], g0[n][e]), (n, e)
+                else:
+                    assert orc.rel_fro(added[e], ref[e]) <= 1e-2, (n, e, orc.rel_fro(added[e], ref[e]))
+        else:
+            assert orc.rel_fro(added, ref) <= 1e-2, n
