@@ -163,6 +163,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(s), "power_w_max": (max(self.power) if self.power else None)}
 
 
+def max_over_ranks(ms, world, device="cuda"):
+    """Replicas only: the job's step time is the slowest replica's."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed(cfg, rank):
+    """Each replica runs the same layer on its own batch."""
+    return cfg.replace(seed=cfg.seed + rank)
+
+
 def stage_flops(cfg):
     """Algorithmic flops per stage per step (S20)."""
     r = cfg.T * cfg.K * cfg.H * cfg.F
@@ -194,7 +210,7 @@ def run_cuda(args, cfg):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks()
     dt = act_dtype(cfg)
-    cfg_r = cfg.replace(seed=cfg.seed + rank)              # each replica gets its own batch
+    cfg_r = replica_seed(cfg, rank)
     lb = LayerBuffers(cfg)
     lb.load(X=wl.gen_X(cfg_r), dY=wl.gen_dY(cfg_r), Wr=wl.gen_Wr(cfg), bias=wl.gen_bias(cfg))
     g = torch.Generator(device="cuda").manual_seed(1234)
@@ -262,10 +278,7 @@ def run_cuda(args, cfg):
     sync_all()
     sampler.stop_flag = True
     ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        tmax = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
+    ms = max_over_ranks(ms, world)
     fl = cfg.flops_fwd_bwd()
     value = world * fl["total"] * args.steps / (ms * 1e-3) / 1e12
 
@@ -282,10 +295,7 @@ def run_cuda(args, cfg):
     e1.record(stream)
     sync_all()
     ms_e2e = e0.elapsed_time(e1)
-    if world > 1:
-        tmax = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_e2e = float(tmax.item())
+    ms_e2e = max_over_ranks(ms_e2e, world)
     act_bytes = cfg.T * cfg.H * (4 if cfg.dtype == wl.DTYPE_FP32 else 2)
     e2e = {"value": world * fl["total"] * args.steps / (ms_e2e * 1e-3) / 1e12, "unit": UNIT,
            "h2d_bytes_per_step": 2 * act_bytes, "d2h_bytes_per_step": 2 * act_bytes, "ms_per_step": ms_e2e / args.steps}
