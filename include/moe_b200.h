@@ -180,6 +180,21 @@ int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const v
                             void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, int32_t* topk_idx,
                             float* topk_w, void* ctx, void* ws, void* stream);
 
+/* The same step, software-pipelined over three caller streams: the H2D copies go to `stream_in`, fwd+bwd to
+ * `stream_compute`, the D2H copies to `stream_out`, ordered by library-owned events, so that consecutive calls overlap
+ * copy-in of step i+1 and copy-out of step i-1 with the compute of step i.  `slot` is 0 or 1 and names which of the
+ * caller's TWO sets of staging buffers (X_dev, dY_dev, Y_dev, dX_dev) this call uses; alternate it between calls.
+ * ctx, ws, weights and gradients are shared by both slots (compute is serial on stream_compute).  The host input
+ * buffers may be changed once stream_in has passed this call's copies; the host outputs are valid once stream_out has.
+ * Host-side state (six events), not thread-safe. */
+int32_t moe_layer_step_host_pipelined(const moe_config_t* cfg, int32_t slot, const void* X_host, const void* dY_host,
+                                      void* Y_host, void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
+                                      const void* Wr, const float* bias, const void* Wg, const void* Wu, const void* Wd,
+                                      const void* Wg_s, const void* Wu_s, const void* Wd_s, void* dWr, void* dWg,
+                                      void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, int32_t* topk_idx,
+                                      float* topk_w, void* ctx, void* ws, void* stream_in, void* stream_compute,
+                                      void* stream_out);
+
 /* Read-only view of buffers inside ctx after moe_layer_fwd (for tests and tracing):
  * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s"}.
  * Writes the byte offset inside ctx and the byte length.  */

@@ -5,7 +5,8 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from . import (make_config, moe_ctx_field, moe_layer_bwd, moe_layer_fwd, moe_layer_step_host, moe_padded_rows,
+from . import (make_config, moe_ctx_field, moe_layer_bwd, moe_layer_fwd, moe_layer_step_host,
+               moe_layer_step_host_pipelined, moe_padded_rows,
                moe_workspace_bytes, moe_ws_field)
 
 
@@ -84,6 +85,19 @@ class LayerBuffers:
                             self.bias, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s, self.Wd_s, self.dWr, self.dWg,
                             self.dWu, self.dWd, self.dWg_s, self.dWu_s, self.dWd_s, self.topk_idx, self.topk_w,
                             self.ctx, self.ws, stream)
+
+    def make_pipeline(self):
+        """Second set of staging buffers and the three streams of moe_layer_step_host_pipelined."""
+        self.stage = [(self.X, self.dY, self.Y, self.dX),
+                      tuple(torch.empty_like(self.X) for _ in range(4))]
+        self.streams = tuple(torch.cuda.Stream() for _ in range(3))
+
+    def step_host_pipelined(self, i, X_host, dY_host, Y_host, dX_host):
+        Xd, dYd, Yd, dXd = self.stage[i & 1]
+        moe_layer_step_host_pipelined(self.ccfg, i & 1, X_host, dY_host, Y_host, dX_host, Xd, dYd, Yd, dXd, self.Wr,
+                                      self.bias, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s, self.Wd_s, self.dWr,
+                                      self.dWg, self.dWu, self.dWd, self.dWg_s, self.dWu_s, self.dWd_s, self.topk_idx,
+                                      self.topk_w, self.ctx, self.ws, *self.streams)
 
     # ---- typed views into ctx / ws ----
     _CTX = {"z": ("f32", lambda c, R: (c.T, c.E)), "counts": ("i32", lambda c, R: (c.E,)),

@@ -142,3 +142,28 @@ def test_delayed_wgrad_overwrite_and_fp32_accumulate(cfg):
                     assert orc.rel_fro(added[e], ref[e]) <= 1e-2, (n, e, orc.rel_fro(added[e], ref[e]))
         else:
             assert orc.rel_fro(added, ref) <= 1e-2, n
+
+
+def test_pipelined_host_step_matches_device_step():
+    """Six overlapping steps through moe_layer_step_host_pipelined on alternating inputs: every step's host outputs
+    equal the plain device step on the same inputs (no buffer of a slot is reused before its consumer has finished)."""
+    import torch
+    from paper_2605_31463_b200.buffers import LayerBuffers, act_dtype
+    cfg = wl.QWEN3_SMALL.replace(row_align=128)
+    inp = gc.gen_inputs(cfg)
+    inp2 = dict(inp, X=wl.gen_X(cfg.replace(seed=5)), dY=wl.gen_dY(cfg.replace(seed=5)))
+    refs = [gc.run_gpu_layer(cfg, inp), gc.run_gpu_layer(cfg, inp2)]
+    lb = LayerBuffers(cfg)
+    lb.load(Wr=inp["Wr"], bias=inp["bias"], W=inp["W"], shared=inp["shared"])
+    lb.make_pipeline()
+    dt = act_dtype(cfg)
+    Xh = [torch.from_numpy(i["X"]).to(dt).pin_memory() for i in (inp, inp2)]
+    dYh = [torch.from_numpy(i["dY"]).to(dt).pin_memory() for i in (inp, inp2)]
+    n = 6
+    Yh = [torch.empty_like(Xh[0]).pin_memory() for _ in range(n)]
+    dXh = [torch.empty_like(Xh[0]).pin_memory() for _ in range(n)]
+    for i in range(n):
+        lb.step_host_pipelined(i, Xh[i % 2], dYh[i % 2], Yh[i], dXh[i])
+    torch.cuda.synchronize()
+    for i in range(n):
+        assert torch.equal(Yh[i], refs[i % 2].Y.cpu()) and torch.equal(dXh[i], refs[i % 2].dX.cpu()), i
