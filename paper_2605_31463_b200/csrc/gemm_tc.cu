@@ -11,7 +11,6 @@
 // Both K-major and MN-major shared-memory operand layouts are used, so the dgrad (weights read
 // "transposed") and wgrad (both operands contracted over rows) need no transposed copies in HBM.
 #include <cuda.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -55,8 +54,7 @@ bool tc_make_map(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t inner,
   const cuuint32_t estr[2] = {1, 1};
   const CUtensorMapDataType dt = elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
   return fn(m, dt, 2, const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 bool tc_make_map3(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t d0, int64_t d1, int64_t d2, int64_t ld, int box0,
@@ -104,7 +102,7 @@ constexpr int TMEM_COLS = 512;
 // kernel parameters
 // ---------------------------------------------------------------------------------------------
 struct TcParams {
-  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, raster, tma_out, acc_f32;
+  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, tma_out, acc_f32;
   int64_t rows_valid;
   const int32_t* mtile;
   const int32_t* offsets;
@@ -136,35 +134,12 @@ __device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_
       tl.row0 = 0;
       tl.nkb = (int)((p.rows_valid + BK - 1) / BK);
     }
-  } else if (p.raster == 0) {
+  } else {
     // n fastest: consecutive CTAs share the 128-row activation tile
     const int mt = (int)(t / p.n_tiles);
     tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
     tl.m0 = mt * BM;
     tl.e = p.mtile ? p.mtile[1 + mt] : 0;
-    tl.nkb = p.nkb;
-    tl.row0 = 0;
-  } else {
-    // expert major, then n, then m fastest: the CTAs that run side by side share the (twice larger) weight tile of
-    // one expert, so L2 serves it once to all of them
-    int e = 0, first = 0, m_cnt;
-    if (p.mtile) {
-      int lo = 0, hi = p.E;   // largest e with (offsets[e] / 128) * n_tiles <= t
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if ((int64_t)(__ldg(p.offsets + mid) >> 7) * p.n_tiles <= t) lo = mid; else hi = mid;
-      }
-      e = lo;
-      first = __ldg(p.offsets + e) >> 7;
-      m_cnt = (__ldg(p.offsets + e + 1) >> 7) - first;
-    } else {
-      m_cnt = (int)((p.rows_valid + BM - 1) / BM);
-    }
-    const int local = (int)(t - (int64_t)first * p.n_tiles);
-    const int nt = local / m_cnt;
-    tl.n0 = nt * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
-    tl.m0 = (first + local - nt * m_cnt) * BM;
-    tl.e = e;
     tl.nkb = p.nkb;
     tl.row0 = 0;
   }
@@ -661,14 +636,6 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.M = c.M;
   p.b_rows = c.b_rows;
   p.a_col0 = c.a_col0;
-  {
-    static int raster = -1;   // tile order of the row-grouped GEMMs: 0 = n fastest (default; measured 2% faster on configs[1]), MOE_TC_RASTER=1 = m fastest within an expert
-    if (raster < 0) {
-      const char* ev = getenv("MOE_TC_RASTER");
-      raster = ev ? atoi(ev) : 0;
-    }
-    p.raster = raster;
-  }
   CUtensorMap ta, tb0, tb1, to;
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
   if (c.mode == TC_FWD_F32 ? ((c.N & 3) || (c.ld0 & 3)) : ((c.N & 7) || (c.ld0 & 7))) return MOE_ERR_UNSUPPORTED;

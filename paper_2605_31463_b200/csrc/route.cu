@@ -94,31 +94,34 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
   }
 
   // ---- R4 top-k: K rounds of arg-max, ties -> lower expert index ----
+  // Keys are mapped to order-preserving unsigned integers (-0 folded into +0 first, so equal floats stay equal);
+  // a round is two hardware warp reductions: redux.max of the lanes' best keys, then redux.min of the expert
+  // indices that hold that key -- exactly the (key desc, index asc) order of the oracle's arg-max.
+  uint32_t ukey[VPT];
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) {
+    const uint32_t u = __float_as_uint(key[s] + 0.0f);
+    ukey[s] = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    if (s * 32 + lane >= p.E) ukey[s] = 0u;          // below every real key (-inf maps to 0x007fffff)
+  }
   int sel_e = 0;
   float sel_z = 0.f;
-  unsigned taken = 0;  // bit s set: this lane's slot s was selected
   for (int j = 0; j < p.K; ++j) {
-    float v = NEG;
-    int e = 0x7fffffff;
+    uint32_t best = 0u;
+    int be = 0x7fffffff;
 #pragma unroll
-    for (int s = 0; s < VPT; ++s) {
-      const int es = s * 32 + lane;
-      const bool ok = es < p.E && !((taken >> s) & 1u);
-      if (ok && (e == 0x7fffffff || key[s] > v)) { v = key[s]; e = es; }
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-      const float ov = __shfl_xor_sync(FULL, v, off);
-      const int oe = __shfl_xor_sync(FULL, e, off);
-      const bool take = (oe != 0x7fffffff) && (e == 0x7fffffff || ov > v || (ov == v && oe < e));
-      if (take) { v = ov; e = oe; }
-    }
+    for (int s = 0; s < VPT; ++s)
+      if (ukey[s] > best) { best = ukey[s]; be = s * 32 + lane; }     // strict >: the lower slot wins a tie inside the lane
+    const uint32_t m = __reduce_max_sync(FULL, best);
+    const int e = (int)__reduce_min_sync(FULL, (best == m && be != 0x7fffffff) ? (unsigned)be : 0x7fffffffu);
     float zsel = 0.f;
 #pragma unroll
     for (int s = 0; s < VPT; ++s)
-      if (s == (e >> 5)) zsel = z[s];
+      if (s == (e >> 5)) {
+        zsel = z[s];
+        if (lane == (e & 31)) ukey[s] = 0u;           // taken
+      }
     zsel = __shfl_sync(FULL, zsel, e & 31);
-    if (lane == (e & 31)) taken |= 1u << (e >> 5);
     if (lane == j) { sel_e = e; sel_z = zsel; }
   }
 
