@@ -84,6 +84,9 @@ int32_t combine(const moe_config_t* c, const void* y, const float* w, const int3
                 const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s);
 int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const float* w, const int32_t* f2p,
                     const int32_t* p2f, const int32_t* offsets, void* dy, float* dw, cudaStream_t s);
+// route.cu: moe_route with an optional second copy of the outputs
+int32_t route_impl(const moe_config_t* c, const float* logits, const float* bias, int32_t* topk_idx, float* topk_w,
+                   int32_t* idx_copy, float* w_copy, void* stream);
 // router.cu
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s);
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,

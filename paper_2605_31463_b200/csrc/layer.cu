@@ -252,9 +252,7 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
   prof_mark(ST_BEGIN, s);
   MOE_CHECK(router_logits(cfg, X, Wr, z, s));                                              // R1
   prof_mark(ST_ROUTER_GEMM, s);
-  MOE_CHECK(moe_route(cfg, z, bias, topk_idx, topk_w, stream));                            // R2..R5
-  MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.idx), topk_idx, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
-  MOE_CUDA(cudaMemcpyAsync(at<char>(ctx, C.w), topk_w, (size_t)cfg->T * cfg->K * 4, cudaMemcpyDeviceToDevice, s));
+  MOE_CHECK(route_impl(cfg, z, bias, topk_idx, topk_w, at<int32_t>(ctx, C.idx), at<float>(ctx, C.w), stream));   // R2..R5
   prof_mark(ST_ROUTE, s);
   MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, p2f, f2p, mtile, at<int32_t>(ws, W.hist), s));  // R6
   prof_mark(ST_MAPS, s);

@@ -18,7 +18,8 @@ struct RouteParams {
 template <int VPT>
 __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* __restrict__ logits,
                                                     const float* __restrict__ bias, int32_t* __restrict__ topk_idx,
-                                                    float* __restrict__ topk_w) {
+                                                    float* __restrict__ topk_w, int32_t* __restrict__ idx_copy,
+                                                    float* __restrict__ w_copy) {
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (t >= p.T) return;
@@ -163,6 +164,10 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
   if (act) {
     topk_idx[(size_t)t * p.K + lane] = sel_e;
     topk_w[(size_t)t * p.K + lane] = wj;
+    if (idx_copy) {                                   // the copy moe_layer_fwd keeps in ctx for the backward
+      idx_copy[(size_t)t * p.K + lane] = sel_e;
+      w_copy[(size_t)t * p.K + lane] = wj;
+    }
   }
 }
 
@@ -170,9 +175,9 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
 
 }  // namespace moe
 
-extern "C" int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
-                             float* topk_w, void* stream) {
-  using namespace moe;
+namespace moe {
+int32_t route_impl(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx, float* topk_w,
+                   int32_t* idx_copy, float* w_copy, void* stream) {
   if (!cfg || !logits || !topk_idx || !topk_w) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(validate(cfg));
   if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
@@ -183,11 +188,17 @@ extern "C" int32_t moe_route(const moe_config_t* cfg, const float* logits, const
   dim3 grid((unsigned)ceil_div(cfg->T, warps)), block(warps * 32);
   cudaStream_t s = as_stream(stream);
   const int vpt = (int)ceil_div(cfg->E, 32);
-  if (vpt <= 1) MOE_LAUNCH(route_kernel<1>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
-  else if (vpt <= 2) MOE_LAUNCH(route_kernel<2>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
-  else if (vpt <= 4) MOE_LAUNCH(route_kernel<4>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
-  else if (vpt <= 8) MOE_LAUNCH(route_kernel<8>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
-  else if (vpt <= 16) MOE_LAUNCH(route_kernel<16>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
-  else MOE_LAUNCH(route_kernel<32>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w);
+  if (vpt <= 1) MOE_LAUNCH(route_kernel<1>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 2) MOE_LAUNCH(route_kernel<2>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 4) MOE_LAUNCH(route_kernel<4>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 8) MOE_LAUNCH(route_kernel<8>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 16) MOE_LAUNCH(route_kernel<16>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  else MOE_LAUNCH(route_kernel<32>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
   return MOE_OK;
+}
+}  // namespace moe
+
+extern "C" int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
+                             float* topk_w, void* stream) {
+  return moe::route_impl(cfg, logits, bias, topk_idx, topk_w, nullptr, nullptr, stream);
 }
