@@ -318,6 +318,54 @@ __device__ __forceinline__ void dgrad_swiglu_chunk(const TcParams& p, const Tile
   }
 }
 
+// TC_DGRAD_SWIGLU chunk with F % 32 == 0: g, u of the chunk (two 32-column x 128-row boxes) were fetched by TMA into the
+// warp group's two 64-byte-swizzled 8 KB boxes; every thread turns its own row into dg, du IN PLACE and the same boxes
+// leave by TMA store.  No per-thread global loads or stores at all.
+__device__ __forceinline__ void dgrad_swiglu_chunk_tma(const TcParams& p, const Tile& tl, int c, uint32_t tacc, uint32_t obuf,
+                                                       int row_in_tile, uint32_t gbar, uint32_t& gphase,
+                                                       const CUtensorMap* tmO, bool issuer, int ch) {
+  uint32_t d[32];
+  tmem_ld32(tacc + c * 32, d);
+  mbar_wait(gbar, gphase);           // g, u of this chunk have landed
+  gphase ^= 1;
+  tmem_ld_wait();
+  const uint32_t rowaddr = obuf + row_in_tile * 64;
+  const int sw = (row_in_tile >> 1) & 3;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const uint32_t ga = rowaddr + ((q ^ sw) << 4), ua = ga + OBUF_BYTES / 2;
+    const uint4 gq = ld_shared_v4(ga), uq = ld_shared_v4(ua);
+    const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
+    uint32_t og[4], ou[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+      const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
+      const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
+      og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
+      ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
+    }
+    st_shared_v4(ga, og[0], og[1], og[2], og[3]);
+    st_shared_v4(ua, ou[0], ou[1], ou[2], ou[3]);
+  }
+  fence_proxy_async();
+  named_bar_sync(1 + ch, 128);
+  if (issuer) {
+    tma_store_3d(tmO, obuf, tl.n0 + c * 32, tl.m0, 0);
+    tma_store_3d(tmO, obuf + OBUF_BYTES / 2, p.F + tl.n0 + c * 32, tl.m0, 0);
+    bulk_commit();
+  }
+}
+
+// issuer thread of a warp group: once the group's previous stores have read the boxes, fetch g, u of chunk c into them
+__device__ __forceinline__ void gu_tma_fetch(const TcParams& p, const Tile& tl, int c, uint32_t obuf, uint32_t gbar,
+                                             const CUtensorMap* tmGU) {
+  bulk_wait_read0();
+  mbar_expect_tx(gbar, OBUF_BYTES);
+  tma_load_3d(obuf, tmGU, gbar, tl.n0 + c * 32, tl.m0, 0);
+  tma_load_3d(obuf + OBUF_BYTES / 2, tmGU, gbar, p.F + tl.n0 + c * 32, tl.m0, 0);
+}
+
 // TC_WGRAD epilogue.  An expert's contraction is short (its row count), so the weight-gradient tiles are bound by
 // how fast 128 x 256 bf16 outputs leave the SM: each 64-column chunk is packed into a 128-byte-swizzled shared-memory
 // box (thread = row, conflict-free 16-byte stores) and written with one TMA store (full 128-byte lines; rows past M
@@ -406,6 +454,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   // barrier addresses: full[s] = bars + 8 s; empty[s] = bars + 8 (STAGES + s); tfull[a] / tempty[a] follow
   const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
   const uint32_t tmem_slot = tempty0 + 16;
+  const uint32_t gbar0 = tempty0 + 24;   // two barriers: g, u boxes of the dgrad-down epilogue groups
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
@@ -420,6 +469,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull0 + 8 * a, 1);
       mbar_init(tempty0 + 8 * a, EPI_WARPS);   // one arrive per epilogue warp
+      mbar_init(gbar0 + 8 * a, 1);
     }
     fence_barrier_init();
   }
@@ -506,7 +556,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int ch = (warp - 2) >> 2;          // which half of the column chunks this warp drains
     const int row_in_tile = lg * 32 + lane;
     int as = 0;
-    uint32_t aphase = 0;
+    uint32_t aphase = 0, gphase = 0;
     Tile tl;
     for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
       const bool have = tl.nkb > 0;
@@ -525,8 +575,27 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
           }
         }
-        GuChunk k[3];
         constexpr int NC = BN / 64;              // chunks per warp: this warp drains columns [ch * 128, ch * 128 + 128)
+        if (p.tma_out) {
+          const bool issuer = (threadIdx.x & 127) == 64;
+          const uint32_t obuf = obuf0 + ch * OBUF_BYTES, gbar = gbar0 + 8 * ch;
+          const int nvalid = min(NC, (p.F - tl.n0 - ch * (BN / 2) + 31) / 32);      // chunks of this group inside F
+          if (issuer && nvalid > 0) gu_tma_fetch(p, tl, ch * NC, obuf, gbar, &tmB1);   // overlaps the rest of the main loop
+          __syncwarp();
+          mbar_wait(tfull0 + 8 * as, aphase);
+          tc_fence_after();
+          for (int i = 0; i < nvalid; ++i) {
+            dgrad_swiglu_chunk_tma(p, tl, ch * NC + i, tacc, obuf, row_in_tile, gbar, gphase, &tmO, issuer, ch);
+            if (issuer && i + 1 < nvalid) gu_tma_fetch(p, tl, ch * NC + i + 1, obuf, gbar, &tmB1);
+            __syncwarp();
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+          if (++as == 2) { as = 0; aphase ^= 1; }
+          continue;
+        }
+        GuChunk k[3];
         gu_load(p, tl, row, row_ok, ch * NC, k[0]);
         gu_load(p, tl, row, row_ok, ch * NC + 1, k[1]);
         mbar_wait(tfull0 + 8 * as, aphase);
@@ -677,6 +746,9 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       }
       if ((c.F & 7) || (c.ldgu & 7)) return MOE_ERR_UNSUPPORTED;
       p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // dg / du boxes of 32 columns must not straddle the [dg|du] boundary
+      if (p.tma_out && !split &&                                                          // saved [g|u] rows, same boxes
+          !tc_make_map3(&tb1, 2, c.gu, 2 * (int64_t)c.F, c.rows_cap, 1, c.ldgu, 32, BM))
+        p.tma_out = 0;
       if (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
       return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
     }
