@@ -237,6 +237,57 @@ __device__ __forceinline__ void epilogue_tile(const TcParams& p, const Tile& tl,
   }
 }
 
+// TC_FWD_SWIGLU epilogue with F % 32 == 0: per 32-column chunk the warp group stages g and u (two 64-byte-swizzled
+// 8 KB boxes) and stores them by TMA, then reuses the first box for a = silu(g) * u.
+__device__ __forceinline__ void pack32_to_box(uint32_t rowaddr, int sw, const uint32_t (&v)[32]) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    st_shared_v4(rowaddr + ((q ^ sw) << 4), pack_bf16(__uint_as_float(v[q * 8 + 0]), __uint_as_float(v[q * 8 + 1])),
+                 pack_bf16(__uint_as_float(v[q * 8 + 2]), __uint_as_float(v[q * 8 + 3])),
+                 pack_bf16(__uint_as_float(v[q * 8 + 4]), __uint_as_float(v[q * 8 + 5])),
+                 pack_bf16(__uint_as_float(v[q * 8 + 6]), __uint_as_float(v[q * 8 + 7])));
+}
+
+__device__ __forceinline__ void fwd_swiglu_tile_tma(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
+                                                    uint32_t obuf, const CUtensorMap* tmGU, const CUtensorMap* tmAo,
+                                                    bool issuer, int ch) {
+  const uint32_t rowaddr = obuf + row_in_tile * 64;
+  const int sw = (row_in_tile >> 1) & 3;
+#pragma unroll 1
+  for (int c = ch; c < BN / 64; c += 2) {
+    if (p.F - (tl.n0 + c * 32) <= 0) break;     // warp-group uniform
+    uint32_t g[32], u[32];
+    tmem_ld32(tacc + c * 32, g);
+    tmem_ld32(tacc + BN / 2 + c * 32, u);
+    tmem_ld_wait();
+    if (issuer) bulk_wait_read0();
+    named_bar_sync(1 + ch, 128);
+    pack32_to_box(rowaddr, sw, g);
+    pack32_to_box(rowaddr + OBUF_BYTES / 2, sw, u);
+    fence_proxy_async();
+    named_bar_sync(1 + ch, 128);
+    if (issuer) {
+      tma_store_3d(tmGU, obuf, tl.n0 + c * 32, tl.m0, 0);
+      tma_store_3d(tmGU, obuf + OBUF_BYTES / 2, p.F + tl.n0 + c * 32, tl.m0, 0);
+      bulk_commit();
+    }
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const float gv = __uint_as_float(g[i]);
+      g[i] = __float_as_uint(gv * fast_sigmoid(gv) * __uint_as_float(u[i]));
+    }
+    if (issuer) bulk_wait_read0();
+    named_bar_sync(1 + ch, 128);
+    pack32_to_box(rowaddr, sw, g);
+    fence_proxy_async();
+    named_bar_sync(1 + ch, 128);
+    if (issuer) {
+      tma_store_3d(tmAo, obuf, tl.n0 + c * 32, tl.m0, 0);
+      bulk_commit();
+    }
+  }
+}
+
 // TC_DGRAD_SWIGLU epilogue: acc = da [128 x 256 columns of F]; dgu = swiglu'(g, u) * da.  The saved g, u of this
 // thread's row are fetched from HBM two 32-column chunks ahead of the TMEM drain (the first two before the
 // accumulator is even complete), so their latency hides behind the main loop and the previous chunk's math.
@@ -444,7 +495,8 @@ __device__ __forceinline__ void wgrad_accum_tile(const TcParams& p, const Tile& 
 template <int MODE>
 __global__ void __launch_bounds__(NTHREADS, 1)
 tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
-               const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmO, const TcParams p) {
+               const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmO,
+               const __grid_constant__ CUtensorMap tmO2, const TcParams p) {
   constexpr bool A_MN = (MODE == TC_WGRAD);
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
   extern __shared__ uint8_t smem_raw[];
@@ -462,6 +514,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     tma_prefetch_desc(&tmB0);
     tma_prefetch_desc(&tmB1);
     tma_prefetch_desc(&tmO);
+    tma_prefetch_desc(&tmO2);
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full0 + 8 * s, 1);
       mbar_init(empty0 + 8 * s, 1);
@@ -617,6 +670,10 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch,
                            MODE == TC_WGRAD ? tl.e : 0);
         }
+      } else if (MODE == TC_FWD_SWIGLU && p.tma_out) {
+        mbar_wait(tfull0 + 8 * as, aphase);
+        tc_fence_after();
+        fwd_swiglu_tile_tma(p, tl, tacc, row_in_tile, obuf0 + ch * OBUF_BYTES, &tmO, &tmO2, (threadIdx.x & 127) == 64, ch);
       } else {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
@@ -631,7 +688,8 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
-    if ((MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU) && (threadIdx.x & 127) == 64)
+    if ((MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_FWD_SWIGLU) &&
+        (threadIdx.x & 127) == 64)
       bulk_wait0();   // all TMA stores complete before the CTA retires
   }
   tc_fence_before();
@@ -653,8 +711,7 @@ bool g_attr_set[6] = {false, false, false, false, false, false};
 
 template <int MODE>
 int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
-               int64_t max_tiles,
-               cudaStream_t s) {
+               int64_t max_tiles, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
   if (!g_attr_set[MODE]) {
     MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
     g_attr_set[MODE] = true;
@@ -665,7 +722,7 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
     MOE_CUDA(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
   }
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(g_sm_count, max_tiles));
-  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, p);
+  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, p);
   return MOE_OK;
 }
 
@@ -727,7 +784,13 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, c.B1, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
-      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, ta, p, max_mtiles * p.n_tiles, s);
+      p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // g / u boxes of 32 columns must not straddle the [g|u] boundary
+      CUtensorMap to2;
+      if (p.tma_out && (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM) ||    // gu [rows, 2F]
+                        !tc_make_map3(&to2, 2, c.out1, c.F, c.rows_cap, 1, c.ld1, 32, BM)))                  // a [rows, F]
+        p.tma_out = 0;
+      if (!p.tma_out) return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, ta, p, max_mtiles * p.n_tiles, s);
+      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s, &to2);
     }
     case TC_DGRAD:
     case TC_DGRAD_SWIGLU: {
