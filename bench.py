@@ -29,10 +29,10 @@ METRIC = "moe_layer_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 NOMINAL = {"bf16_tflops": 2250.0, "hbm_gbs": 8000.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each GEMM stage's kernel, from the `ncu --set full` capture
-# summarised in profiles/r1c_step_full.md (configs[1] only; other workloads report traffic = null).
-NCU_TRAFFIC = {"qwen3_30b_a3b_like": {"gemm1_swiglu": 1.112e9 + 314.4e6, "gemm2": 0.517e9 + 272.1e6,
-                                      "dgrad_down_swiglu": 1.171e9 + 198.9e6, "dgrad_gateup": 1.034e9 + 287.2e6,
-                                      "wgrad": 0.419e9 + 360.4e6}}
+# summarised in profiles/r1e_step_full.md (configs[1] only; other workloads report traffic = null).
+NCU_TRAFFIC = {"qwen3_30b_a3b_like": {"gemm1_swiglu": 1.111e9 + 320.8e6, "gemm2": 0.517e9 + 274.1e6,
+                                      "dgrad_down_swiglu": 1.205e9 + 203.8e6, "dgrad_gateup": 1.034e9 + 287.5e6,
+                                      "wgrad": 0.419e9 + 360.1e6}}
 
 
 def load_peaks():
