@@ -28,11 +28,21 @@ import workloads as wl  # noqa: E402
 METRIC = "moe_layer_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 NOMINAL = {"bf16_tflops": 2250.0, "hbm_gbs": 8000.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of each GEMM stage's kernel, from the `ncu --set full` capture
-# summarised in profiles/r1e_step_full.md (configs[1] only; other workloads report traffic = null).
-NCU_TRAFFIC = {"qwen3_30b_a3b_like": {"gemm1_swiglu": 1.111e9 + 320.8e6, "gemm2": 0.517e9 + 274.1e6,
-                                      "dgrad_down_swiglu": 1.205e9 + 203.8e6, "dgrad_gateup": 1.034e9 + 287.5e6,
-                                      "wgrad": 0.419e9 + 360.1e6}}
+NOMINAL_FP8_OVER_BF16 = 2.0   # B200_PROFILING.md: 4.5 vs 2.25 PFLOP/s dense; the fp8 peak is ASSUMED = measured bf16 x 2
+
+
+def load_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's kernel, read from profiles/traffic.json
+    (written by `python -m paper_2605_31463_b200.ncu_summary` from an `ncu --set full` capture; it names the capture).
+    Returns ({stage: bytes}, source string) or ({}, None) when no capture of this workload is tracked."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        rec = json.load(open(path)).get(workload)
+    except (OSError, ValueError):
+        rec = None
+    if not rec:
+        return {}, None
+    return rec.get("stages", {}), rec.get("source")
 
 
 def load_peaks():
@@ -188,12 +198,29 @@ def stage_flops(cfg):
 
 
 def stage_bytes(cfg):
-    """Algorithmic HBM bytes per stage per step."""
+    """Algorithmic HBM bytes per stage per step: every operand read once, every result written once.
+    GEMM stages: activations at 2 bytes (fp8 fprop/dgrad operands at 1 byte + fp32 scales), weights once per step."""
     b = 4 if cfg.dtype == wl.DTYPE_FP32 else 2
-    T, H, E, K, TK = cfg.T, cfg.H, cfg.E, cfg.K, cfg.T * cfg.K
+    T, H, E, K, F, TK = cfg.T, cfg.H, cfg.E, cfg.K, cfg.F, cfg.T * cfg.K
+    fp8 = cfg.dtype == wl.DTYPE_FP8
+    ab = 1 if fp8 else b                       # bytes per element of an fprop / dgrad GEMM operand
+    sc = (lambda rows, cols: rows * (cols // 128) * 4) if fp8 else (lambda rows, cols: 0)
+    W = E * H * F
     return {"route": T * E * 4 + TK * 8, "maps": 3 * TK * 4, "permute": T * H * b + TK * H * b + TK * 4,
             "combine": TK * H * b + T * H * b + TK * 8, "combine_bwd": 2 * TK * H * b + T * H * b + TK * 12,
-            "dx_combine": TK * H * b + T * H * b + TK * 4}
+            "dx_combine": TK * H * b + T * H * b + TK * 4,
+            "gemm1_swiglu": TK * H * ab + sc(TK, H) + 2 * W * ab + TK * 3 * F * b,      # Xp, Wg, Wu -> gu, a
+            "gemm2": TK * F * ab + sc(TK, F) + W * ab + TK * H * b,                      # a, Wd -> y
+            "dgrad_down_swiglu": TK * H * ab + sc(TK, H) + W * ab + TK * 2 * F * b + TK * 2 * F * b,   # dy, Wd, gu -> dgu
+            "dgrad_gateup": TK * 2 * F * ab + sc(TK, 2 * F) + 2 * W * ab + TK * H * b,   # dgu, Wg, Wu -> dXp
+            "wgrad": TK * (2 * H + 3 * F) * b + 3 * W * b}                               # dy, a, dgu, Xp -> dWd, dWg, dWu
+
+
+def roof(flops, byts, sec, peak_tflops, peak_gbs):
+    """Roofline of one stage: which roof binds (the larger of flops/peak and bytes/peak) and the achieved fraction of it."""
+    t_tensor, t_hbm = flops / (peak_tflops * 1e12), byts / (peak_gbs * 1e9)
+    bound = "tensor" if t_tensor >= t_hbm else "hbm"
+    return bound, max(t_tensor, t_hbm) / sec
 
 
 def run_cuda(args, cfg):
@@ -328,10 +355,11 @@ def run_cuda(args, cfg):
     e1.record(stream)
     sync_all()
     ms_serial = max_over_ranks(e0.elapsed_time(e1), world)
+    lb.close_pipeline()
     act_bytes = cfg.T * cfg.H * (4 if cfg.dtype == wl.DTYPE_FP32 else 2)
     e2e = {"value": world * fl["total"] * args.steps / (ms_e2e * 1e-3) / 1e12, "unit": UNIT,
            "h2d_bytes_per_step": 2 * act_bytes, "d2h_bytes_per_step": 2 * act_bytes, "ms_per_step": ms_e2e / args.steps,
-           "api": "moe_layer_step_host_pipelined (3 streams, 2 staging slots, pinned host buffers)",
+           "api": "moe_layer_step_host_pipelined (3 streams, 2 staging slots, pinned host buffers, caller-owned pipeline object)",
            "serial_value": world * fl["total"] * args.steps / (ms_serial * 1e-3) / 1e12,
            "serial_ms_per_step": ms_serial / args.steps}
 
@@ -340,33 +368,70 @@ def run_cuda(args, cfg):
             dist.destroy_process_group()
         return
     # ---- stage table: TFLOP/s for the GEMMs, GB/s for the HBM-bound movers ----
+    # Which bf16 peak applies is decided from the evidence of THIS run (B200_PROFILING.md: burst for a kernel timed
+    # alone or in a short region at full clock, sustained for seconds-long loops under the power cap): a timed region
+    # shorter than 1 s, or a sampled median SM clock above 0.9 x max, is the burst regime.  Both fractions are printed.
+    clocks = sampler.result()
+    burst = (ms * 1e-3 < 1.0) or bool(clocks["sm_mhz"] and clocks["sm_max_mhz"] and clocks["sm_mhz"] > 0.9 * clocks["sm_max_mhz"])
+    regime = "burst" if burst else "sustained"
+    bf16_peak = peaks["bf16_burst"] if burst else peaks["bf16_sustained"]
     sf, sb = stage_flops(cfg), stage_bytes(cfg)
+    traffic, traffic_src = load_traffic(cfg.name)
+    gemm_names = ("gemm1_swiglu", "gemm2", "dgrad_down_swiglu", "dgrad_gateup", "wgrad")
+
+    def stage_peak(name):          # fprop and dgrad of an fp8 config run on e4m3 codes, its wgrad on bf16
+        fp8_stage = cfg.dtype == wl.DTYPE_FP8 and name in gemm_names and name != "wgrad"
+        return bf16_peak * (NOMINAL_FP8_OVER_BF16 if fp8_stage else 1.0)
+
     for name, st in stages.items():
         sec = st["ms_per_step"] * 1e-3
         if name in sf and sf[name] and sec > 0:
             st["tflops"] = sf[name] / sec / 1e12
-            st["frac_measured_sustained"] = st["tflops"] / peaks["bf16_sustained"]
-            st["frac_nominal"] = st["tflops"] / NOMINAL["bf16_tflops"]
+            mult = stage_peak(name) / bf16_peak
+            st["frac_measured_burst"] = st["tflops"] / (peaks["bf16_burst"] * mult)
+            st["frac_measured_sustained"] = st["tflops"] / (peaks["bf16_sustained"] * mult)
+            st["frac_nominal"] = st["tflops"] / (NOMINAL["bf16_tflops"] * mult)
         if name in sb and sec > 0:
             st["gbs"] = sb[name] / sec / 1e9
-            st["frac_measured"] = st["gbs"] / peaks["hbm_gbs"]
-            st["frac_nominal"] = st["gbs"] / NOMINAL["hbm_gbs"]
-    gemm_stages = [n for n in ("gemm1_swiglu", "gemm2", "dgrad_down_swiglu", "dgrad_gateup", "wgrad") if n in stages]
-    roofline = None
+            st["frac_measured_hbm"] = st["gbs"] / peaks["hbm_gbs"]
+            st["frac_nominal_hbm"] = st["gbs"] / NOMINAL["hbm_gbs"]
+        if name in sf and name in sb and sf[name] and sec > 0:
+            st["bound"], st["frac_of_binding_roof"] = roof(sf[name], sb[name], sec, stage_peak(name), peaks["hbm_gbs"])
+    gemm_stages = [n for n in gemm_names if n in stages]
+    roofline = gemm_all = None
     if gemm_stages:
+        # the dominant kernel = the GEMM stage with the most time; its roof is whichever of tensor / hbm binds (SURVEY.md
+        # §8d: configs[2], [3] stream 22.5 / 11.3 GB of weights per pass and are HBM-bound; configs[1], [4] tensor-bound)
         dom = max(gemm_stages, key=lambda n: stages[n]["ms_per_step"])
         st = stages[dom]
         nl = 3 if dom == "wgrad" else 1
-        tc = "tflops" in st and cfg.dtype != wl.DTYPE_FP32
-        fp8_stage = cfg.dtype == wl.DTYPE_FP8 and dom != "wgrad"     # fprop and dgrad run on e4m3 codes, wgrad on bf16
-        peak = peaks["bf16_sustained"] * (2.0 if fp8_stage else 1.0)  # fp8 peak = measured bf16 x the nominal 2:1 ratio
-        roofline = {"bound": "tensor" if tc else "alu", "kernel": dom, "achieved": st.get("tflops"),
-                    "peak": peak, "unit": "TFLOP/s",
-                    "frac": (st["tflops"] / peak) if "tflops" in st else None,
-                    "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(dom), "traffic_unit": "bytes per launch (ncu dram read+write)",
-                    "algorithmic_flops_per_launch": sf[dom] / nl, "launches_per_step": nl, "ms_per_launch": st["ms_per_step"] / nl,
-                    "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
-                    "frac_nominal_2250": st.get("frac_nominal")}
+        sec = st["ms_per_step"] * 1e-3
+        if cfg.dtype == wl.DTYPE_FP32:
+            roofline = {"bound": "alu", "kernel": dom, "achieved": st.get("tflops"), "peak": None, "unit": "TFLOP/s", "frac": None,
+                        "traffic": None, "note": "configs[0] runs the fp32 CUDA-core path (parity case, not a bench workload)"}
+        else:
+            bound, frac = roof(sf[dom], sb[dom], sec, stage_peak(dom), peaks["hbm_gbs"])
+            tensor = bound == "tensor"
+            roofline = {"bound": bound, "kernel": dom,
+                        "achieved": st["tflops"] if tensor else st["gbs"],
+                        "peak": stage_peak(dom) if tensor else peaks["hbm_gbs"], "unit": "TFLOP/s" if tensor else "GB/s",
+                        "frac": frac, "traffic": traffic.get(dom), "traffic_unit": "bytes per launch (ncu dram read+write)",
+                        "traffic_source": traffic_src,
+                        "algorithmic_flops_per_launch": sf[dom] / nl, "algorithmic_bytes_per_launch": sb[dom] / nl,
+                        "launches_per_step": nl, "ms_per_launch": st["ms_per_step"] / nl,
+                        "peak_regime": regime, "peak_source": peaks["source"] + f", {regime} bf16"
+                        + (" x 2 (assumed fp8:bf16 ratio, not measured)" if stage_peak(dom) != bf16_peak else ""),
+                        "frac_tensor_burst": st["frac_measured_burst"], "frac_tensor_sustained": st["frac_measured_sustained"],
+                        "frac_tensor_nominal": st["frac_nominal"], "frac_hbm_measured": st["frac_measured_hbm"]}
+        # the aggregate the north_star's ">= 60 % of dense bf16 peak for the grouped GEMMs" is quoted on
+        tsec = sum(stages[n]["ms_per_step"] for n in gemm_stages) * 1e-3
+        tfl = sum(sf[n] for n in gemm_stages)
+        if tsec > 0:
+            gemm_all = {"flops": tfl, "ms": tsec * 1e3, "tflops": tfl / tsec / 1e12,
+                        "frac_measured_burst": tfl / tsec / 1e12 / peaks["bf16_burst"],
+                        "frac_measured_sustained": tfl / tsec / 1e12 / peaks["bf16_sustained"],
+                        "frac_nominal_2250": tfl / tsec / 1e12 / NOMINAL["bf16_tflops"], "stages": gemm_stages,
+                        "note": "bf16 denominators; an fp8 config's fprop/dgrad stages have twice that peak"}
     rp = [stages[n]["ms_per_step"] for n in ("route", "maps", "permute") if n in stages]
     route_permute = None
     if len(rp) == 3:
@@ -387,9 +452,10 @@ def run_cuda(args, cfg):
                        "F_shared": cfg.F_shared, "row_align": cfg.row_align, "parallelism": f"replicas x{world}",
                        "l2": "not flushed: each step streams > 1 GB of weights and activations, larger than the 126 MB L2",
                        "inputs": "X, dY, Wr, bias from workloads (Philox, seed 0); expert weights torch.randn on device"},
-            "flops_per_step": fl, "frac_of_measured_bf16_sustained": value / world / peaks["bf16_sustained"],
+            "flops_per_step": fl, "frac_of_measured_bf16_burst": value / world / peaks["bf16_burst"],
+            "frac_of_measured_bf16_sustained": value / world / peaks["bf16_sustained"],
             "frac_of_nominal_bf16_2250": value / world / NOMINAL["bf16_tflops"],
-            "clocks": sampler.result(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "gemm_all": gemm_all,
             "route_permute": route_permute, "stages": stages, "cpu_baseline": cpu, "peaks": peaks}
     print(json.dumps(line))
     if world > 1:

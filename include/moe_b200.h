@@ -9,12 +9,16 @@
  *
  * Conventions (all entry points)
  *  - Every pointer is a DEVICE pointer owned by the caller unless its name ends in `_host`.
- *    The library allocates no device memory and keeps no global state besides lazily resolved
- *    driver entry points.  Scratch comes from the caller (`ws`), sized by moe_workspace_bytes.
+ *    The library allocates no device memory.  Its only process-wide state is host-side and per device: lazily
+ *    resolved driver entry points, "function attribute already raised" flags and the SM count, each indexed by
+ *    the current device, plus the optional profiling marks of moe_profile_*.  Scratch comes from the caller
+ *    (`ws`), sized by moe_workspace_bytes; the pipelined host step keeps its events in a caller-owned object.
  *  - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream);
  *    calls return without synchronising.  Per-expert counts never visit the host.
  *  - Row-major, innermost dimension contiguous, base pointers 16-byte aligned.
- *  - Return value: MOE_OK or a negative moe_status; on error nothing has been enqueued.
+ *  - Return value: MOE_OK or a negative moe_status.  INVALID_ARG and UNSUPPORTED are decided before the first
+ *    launch (the layer calls check every stage's limits up front), so on those nothing has been enqueued and
+ *    no output buffer has been touched; MOE_ERR_CUDA (a failed launch or runtime call) can occur mid-way.
  *    No exceptions, no aborts, no printing.  Inputs must be finite.
  *  - Activation / weight element type follows cfg->dtype: 0 = fp32, 1 = bf16, 2 = bf16 I/O with
  *    e4m3 block-scaled expert GEMMs.  Logits, gating weights and their gradients are always fp32.
@@ -181,19 +185,24 @@ int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const v
                             float* topk_w, void* ctx, void* ws, void* stream);
 
 /* The same step, software-pipelined over three caller streams: the H2D copies go to `stream_in`, fwd+bwd to
- * `stream_compute`, the D2H copies to `stream_out`, ordered by library-owned events, so that consecutive calls overlap
- * copy-in of step i+1 and copy-out of step i-1 with the compute of step i.  `slot` is 0 or 1 and names which of the
- * caller's TWO sets of staging buffers (X_dev, dY_dev, Y_dev, dX_dev) this call uses; alternate it between calls.
- * ctx, ws, weights and gradients are shared by both slots (compute is serial on stream_compute).  The host input
- * buffers may be changed once stream_in has passed this call's copies; the host outputs are valid once stream_out has.
- * Host-side state (six events), not thread-safe. */
-int32_t moe_layer_step_host_pipelined(const moe_config_t* cfg, int32_t slot, const void* X_host, const void* dY_host,
-                                      void* Y_host, void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
-                                      const void* Wr, const float* bias, const void* Wg, const void* Wu, const void* Wd,
-                                      const void* Wg_s, const void* Wu_s, const void* Wd_s, void* dWr, void* dWg,
-                                      void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, int32_t* topk_idx,
-                                      float* topk_w, void* ctx, void* ws, void* stream_in, void* stream_compute,
-                                      void* stream_out);
+ * `stream_compute`, the D2H copies to `stream_out`, ordered by the events of a caller-owned pipeline object, so that
+ * consecutive calls overlap copy-in of step i+1 and copy-out of step i-1 with the compute of step i.
+ *   moe_pipeline_create:  makes the object (six events, timing disabled) on the CURRENT device; *pipeline receives it.
+ *   moe_pipeline_destroy: destroys it; the caller must have synchronised the three streams first.
+ * `slot` is 0 or 1 and names which of the caller's TWO sets of staging buffers (X_dev, dY_dev, Y_dev, dX_dev) this call
+ * uses; alternate it between calls.  ctx, ws, weights and gradients are shared by both slots (compute is serial on
+ * stream_compute).  The host input buffers may be changed once stream_in has passed this call's copies; the host
+ * outputs are valid once stream_out has.  One pipeline object serves one (device, stream triple, buffer set); it is not
+ * thread-safe.  INVALID_ARG if `pipeline` is not a live object of the current device. */
+int32_t moe_pipeline_create(void** pipeline);
+int32_t moe_pipeline_destroy(void* pipeline);
+int32_t moe_layer_step_host_pipelined(void* pipeline, const moe_config_t* cfg, int32_t slot, const void* X_host,
+                                      const void* dY_host, void* Y_host, void* dX_host, void* X_dev, void* dY_dev,
+                                      void* Y_dev, void* dX_dev, const void* Wr, const float* bias, const void* Wg,
+                                      const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
+                                      void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s,
+                                      int32_t* topk_idx, float* topk_w, void* ctx, void* ws, void* stream_in,
+                                      void* stream_compute, void* stream_out);
 
 /* Read-only view of buffers inside ctx after moe_layer_fwd (for tests and tracing):
  * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s"}.
@@ -207,7 +216,8 @@ int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_off
  * device time and the number of recorded segments of one stage since the last moe_profile_enable call.  Stages:
  * "router_gemm","route","maps","permute","gemm1_swiglu","gemm2","combine","combine_bwd","dgrad_down_swiglu",
  * "dgrad_gateup","wgrad","router_bwd","dx_combine","shared_fwd","shared_bwd","quant".  Host-side state, not
- * thread-safe; at most 8192 marks are kept between two enable calls. */
+ * thread-safe; at most 8192 marks are kept between two enable calls -- past that moe_profile_stage_ms returns
+ * MOE_ERR_WORKSPACE instead of a truncated total. */
 int32_t moe_profile_enable(int32_t on);
 int32_t moe_profile_stage_ms(const char* stage, double* total_ms, int64_t* segments);
 

@@ -64,7 +64,9 @@ _SIGNATURES = {
     "moe_layer_bwd": (_I32, [_CFG] + [_P] * 20),
     "moe_layer_wgrad": (_I32, [_CFG] + [_P] * 10 + [_I32, _P]),
     "moe_layer_step_host": (_I32, [_CFG] + [_P] * 28),
-    "moe_layer_step_host_pipelined": (_I32, [_CFG, _I32] + [_P] * 30),
+    "moe_pipeline_create": (_I32, [C.POINTER(C.c_void_p)]),
+    "moe_pipeline_destroy": (_I32, [_P]),
+    "moe_layer_step_host_pipelined": (_I32, [_P, _CFG, _I32] + [_P] * 30),
     "moe_ctx_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
     "moe_ws_field": (_I32, [_CFG, C.c_char_p, _SZP, _SZP]),
     "moe_profile_enable": (_I32, [_I32]),
@@ -251,11 +253,21 @@ def moe_layer_step_host(cfg, X_host, dY_host, Y_host, dX_host, X_dev, dY_dev, Y_
            "moe_layer_step_host")
 
 
-def moe_layer_step_host_pipelined(cfg, slot, X_host, dY_host, Y_host, dX_host, X_dev, dY_dev, Y_dev, dX_dev, Wr, bias, Wg,
+def moe_pipeline_create():
+    h = C.c_void_p(None)
+    _check(lib().moe_pipeline_create(C.byref(h)), "moe_pipeline_create")
+    return h
+
+
+def moe_pipeline_destroy(pipeline):
+    _check(lib().moe_pipeline_destroy(pipeline), "moe_pipeline_destroy")
+
+
+def moe_layer_step_host_pipelined(pipeline, cfg, slot, X_host, dY_host, Y_host, dX_host, X_dev, dY_dev, Y_dev, dX_dev, Wr, bias, Wg,
                                   Wu, Wd, Wg_s, Wu_s, Wd_s, dWr, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, topk_idx, topk_w, ctx,
                                   ws, stream_in, stream_compute, stream_out):
     args = [X_host, dY_host, Y_host, dX_host, X_dev, dY_dev, Y_dev, dX_dev, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s,
             dWr, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, topk_idx, topk_w, ctx, ws]
-    _check(lib().moe_layer_step_host_pipelined(C.byref(make_config(cfg)), int(slot), *[_ptr(a) for a in args],
+    _check(lib().moe_layer_step_host_pipelined(pipeline, C.byref(make_config(cfg)), int(slot), *[_ptr(a) for a in args],
                                                _stream(stream_in), _stream(stream_compute), _stream(stream_out)),
            "moe_layer_step_host_pipelined")

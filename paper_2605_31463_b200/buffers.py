@@ -6,7 +6,7 @@ import numpy as np
 import torch
 
 from . import (make_config, moe_ctx_field, moe_layer_bwd, moe_layer_fwd, moe_layer_step_host,
-               moe_layer_step_host_pipelined, moe_padded_rows,
+               moe_layer_step_host_pipelined, moe_padded_rows, moe_pipeline_create, moe_pipeline_destroy,
                moe_workspace_bytes, moe_ws_field)
 
 
@@ -91,10 +91,17 @@ class LayerBuffers:
         self.stage = [(self.X, self.dY, self.Y, self.dX),
                       tuple(torch.empty_like(self.X) for _ in range(4))]
         self.streams = tuple(torch.cuda.Stream() for _ in range(3))
+        self.pipeline = moe_pipeline_create()
+
+    def close_pipeline(self):
+        if getattr(self, "pipeline", None) is not None:
+            torch.cuda.synchronize()
+            moe_pipeline_destroy(self.pipeline)
+            self.pipeline = None
 
     def step_host_pipelined(self, i, X_host, dY_host, Y_host, dX_host):
         Xd, dYd, Yd, dXd = self.stage[i & 1]
-        moe_layer_step_host_pipelined(self.ccfg, i & 1, X_host, dY_host, Y_host, dX_host, Xd, dYd, Yd, dXd, self.Wr,
+        moe_layer_step_host_pipelined(self.pipeline, self.ccfg, i & 1, X_host, dY_host, Y_host, dX_host, Xd, dYd, Yd, dXd, self.Wr,
                                       self.bias, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s, self.Wd_s, self.dWr,
                                       self.dWg, self.dWu, self.dWd, self.dWg_s, self.dWu_s, self.dWd_s, self.topk_idx,
                                       self.topk_w, self.ctx, self.ws, *self.streams)

@@ -1,4 +1,5 @@
 // Public grouped-GEMM entry points and the host-buffer step (include/moe_b200.h).
+#include <new>
 #include <string.h>
 
 #include "fp8.cuh"
@@ -78,7 +79,7 @@ extern "C" int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_ho
                                        int32_t* topk_idx, float* topk_w, void* ctx, void* ws, void* stream) {
   if (!cfg || !X_host || !dY_host || !Y_host || !dX_host || !X_dev || !dY_dev || !Y_dev || !dX_dev)
     return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(validate(cfg));
+  MOE_CHECK(layer_preflight(cfg, true));
   cudaStream_t s = as_stream(stream);
   const size_t bytes = (size_t)cfg->T * cfg->H * elem_bytes(cfg);
   MOE_CUDA(cudaMemcpyAsync(X_dev, X_host, bytes, cudaMemcpyHostToDevice, s));
@@ -93,38 +94,75 @@ extern "C" int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_ho
 
 // Pipelined host-buffer step: H2D of the step's inputs, fwd+bwd and D2H of its results run on three caller streams
 // so that copy-in of step i+1 and copy-out of step i-1 overlap the compute of step i.  `slot` (0/1) selects which of
-// the caller's two sets of device staging buffers this step uses; six lazily created events (library-owned, timing
-// disabled) order the reuse of a slot: copy-in waits for the compute that last read the slot's inputs, compute waits
-// for the copy-out that last read the slot's outputs.
+// the caller's two sets of device staging buffers this step uses; the six events that order the reuse of a slot
+// (copy-in waits for the compute that last read the slot's inputs, compute waits for the copy-out that last read the
+// slot's outputs) live in a CALLER-OWNED pipeline object created on the caller's current device, so the library
+// itself holds no state for this call.
 namespace {
-cudaEvent_t g_pipe_ev[2][3];
-bool g_pipe_ev_ok = false;
-bool g_pipe_used[2] = {false, false};
+struct Pipeline {
+  uint32_t magic;
+  int device;
+  cudaEvent_t ev[2][3];
+  bool used[2];
+};
+constexpr uint32_t PIPE_MAGIC = 0x4d6f4550u;   // "MoEP"
 }  // namespace
 
+extern "C" int32_t moe_pipeline_create(void** pipeline) {
+  if (!pipeline) return MOE_ERR_INVALID_ARG;
+  *pipeline = nullptr;
+  const int dev = current_device();
+  if (dev < 0) return MOE_ERR_CUDA;
+  Pipeline* p = new (std::nothrow) Pipeline();
+  if (!p) return MOE_ERR_WORKSPACE;
+  p->magic = PIPE_MAGIC;
+  p->device = dev;
+  p->used[0] = p->used[1] = false;
+  int made = 0;
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 3; ++j, ++made)
+      if (cudaEventCreateWithFlags(&p->ev[i][j], cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        for (int k = 0; k < made; ++k) cudaEventDestroy(p->ev[k / 3][k % 3]);
+        delete p;
+        return MOE_ERR_CUDA;
+      }
+  *pipeline = p;
+  return MOE_OK;
+}
+
+extern "C" int32_t moe_pipeline_destroy(void* pipeline) {
+  Pipeline* p = static_cast<Pipeline*>(pipeline);
+  if (!p || p->magic != PIPE_MAGIC) return MOE_ERR_INVALID_ARG;
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 3; ++j) cudaEventDestroy(p->ev[i][j]);
+  cudaGetLastError();
+  p->magic = 0;
+  delete p;
+  return MOE_OK;
+}
+
 extern "C" int32_t moe_layer_step_host_pipelined(
-    const moe_config_t* cfg, int32_t slot, const void* X_host, const void* dY_host, void* Y_host, void* dX_host,
-    void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev, const void* Wr, const float* bias, const void* Wg,
+    void* pipeline, const moe_config_t* cfg, int32_t slot, const void* X_host, const void* dY_host, void* Y_host,
+    void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev, const void* Wr, const float* bias, const void* Wg,
     const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s, void* dWr, void* dWg, void* dWu,
     void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
     void* stream_in, void* stream_compute, void* stream_out) {
+  Pipeline* pl = static_cast<Pipeline*>(pipeline);
+  if (!pl || pl->magic != PIPE_MAGIC) return MOE_ERR_INVALID_ARG;
   if (!cfg || !X_host || !dY_host || !Y_host || !dX_host || !X_dev || !dY_dev || !Y_dev || !dX_dev || slot < 0 || slot > 1)
     return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(validate(cfg));
-  if (!g_pipe_ev_ok) {
-    for (int i = 0; i < 2; ++i)
-      for (int j = 0; j < 3; ++j) MOE_CUDA(cudaEventCreateWithFlags(&g_pipe_ev[i][j], cudaEventDisableTiming));
-    g_pipe_ev_ok = true;
-  }
+  MOE_CHECK(layer_preflight(cfg, true));
+  if (current_device() != pl->device) return MOE_ERR_INVALID_ARG;   // the events belong to the device they were made on
   cudaStream_t si = as_stream(stream_in), sc = as_stream(stream_compute), so = as_stream(stream_out);
-  cudaEvent_t ev_in = g_pipe_ev[slot][0], ev_comp = g_pipe_ev[slot][1], ev_out = g_pipe_ev[slot][2];
+  cudaEvent_t ev_in = pl->ev[slot][0], ev_comp = pl->ev[slot][1], ev_out = pl->ev[slot][2];
   const size_t bytes = (size_t)cfg->T * cfg->H * elem_bytes(cfg);
-  if (g_pipe_used[slot]) MOE_CUDA(cudaStreamWaitEvent(si, ev_comp, 0));
+  if (pl->used[slot]) MOE_CUDA(cudaStreamWaitEvent(si, ev_comp, 0));
   MOE_CUDA(cudaMemcpyAsync(X_dev, X_host, bytes, cudaMemcpyHostToDevice, si));
   MOE_CUDA(cudaMemcpyAsync(dY_dev, dY_host, bytes, cudaMemcpyHostToDevice, si));
   MOE_CUDA(cudaEventRecord(ev_in, si));
   MOE_CUDA(cudaStreamWaitEvent(sc, ev_in, 0));
-  if (g_pipe_used[slot]) MOE_CUDA(cudaStreamWaitEvent(sc, ev_out, 0));
+  if (pl->used[slot]) MOE_CUDA(cudaStreamWaitEvent(sc, ev_out, 0));
   MOE_CHECK(moe_layer_fwd(cfg, X_dev, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, Y_dev, topk_idx, topk_w, ctx, ws, stream_compute));
   MOE_CHECK(moe_layer_bwd(cfg, dY_dev, X_dev, Wr, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, dX_dev, dWr, dWg, dWu, dWd, dWg_s,
                           dWu_s, dWd_s, ws, stream_compute));
@@ -133,6 +171,6 @@ extern "C" int32_t moe_layer_step_host_pipelined(
   MOE_CUDA(cudaMemcpyAsync(Y_host, Y_dev, bytes, cudaMemcpyDeviceToHost, so));
   MOE_CUDA(cudaMemcpyAsync(dX_host, dX_dev, bytes, cudaMemcpyDeviceToHost, so));
   MOE_CUDA(cudaEventRecord(ev_out, so));
-  g_pipe_used[slot] = true;
+  pl->used[slot] = true;
   return MOE_OK;
 }

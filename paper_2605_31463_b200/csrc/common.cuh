@@ -50,6 +50,19 @@ inline int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 inline int64_t ceil_div(int64_t x, int64_t a) { return (x + a - 1) / a; }
 
 int32_t validate(const moe_config_t* c);
+// Every limit of every stage of moe_layer_fwd / bwd / wgrad for this config, checked BEFORE the first launch, so that
+// an UNSUPPORTED layer call enqueues nothing (include/moe_b200.h conventions).  Includes validate().
+int32_t layer_preflight(const moe_config_t* c, bool backward);
+
+// Lazily filled per-device caches (function attributes, SM counts) are indexed by the CURRENT device, so a process
+// that drives several GPUs (or several contexts) through the library gets each device set up once.
+constexpr int MAX_DEVICES = 64;
+inline int current_device() {
+  int d = 0;
+  if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); return -1; }
+  return (d >= 0 && d < MAX_DEVICES) ? d : -1;
+}
+int device_sm_count();   // SM count of the current device (cached per device); <= 0 on error
 inline int64_t padded_rows(const moe_config_t* c) {
   int64_t tk = (int64_t)c->T * c->K;
   if (c->row_align <= 1) return tk;

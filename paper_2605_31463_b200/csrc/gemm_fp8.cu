@@ -305,14 +305,16 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // ---------------------------------------------------------------------------------------------
 // host
 // ---------------------------------------------------------------------------------------------
-bool g_attr_set[4] = {false, false, false, false};
+bool g_attr_set[MAX_DEVICES][4];   // per device
 
 template <int MODE>
 int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const F8Params& p, int64_t max_tiles,
                cudaStream_t s) {
-  if (!g_attr_set[MODE]) {
+  const int dev = current_device();
+  if (dev < 0) return MOE_ERR_CUDA;
+  if (!g_attr_set[dev][MODE]) {
     MOE_CUDA(cudaFuncSetAttribute(f8_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    g_attr_set[MODE] = true;
+    g_attr_set[dev][MODE] = true;
   }
   const int sms = tc_sm_count();
   if (sms <= 0) return MOE_ERR_CUDA;

@@ -72,14 +72,7 @@ bool tc_make_map3(CUtensorMap* m, int elem_bytes, const void* ptr, int64_t d0, i
             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int tc_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
-  }
-  return n;
-}
+int tc_sm_count() { return device_sm_count(); }
 
 namespace {
 
@@ -706,22 +699,20 @@ bool make_map(CUtensorMap* m, const void* ptr, int64_t inner, int64_t outer, int
   return tc_make_map(m, 2, ptr, inner, outer, ld, BK, box_outer);
 }
 
-int g_sm_count = 0;
-bool g_attr_set[6] = {false, false, false, false, false, false};
+bool g_attr_set[MAX_DEVICES][6];   // per device: cudaFuncAttributeMaxDynamicSharedMemorySize raised for tc_gemm_kernel<MODE>
 
 template <int MODE>
 int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
                int64_t max_tiles, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
-  if (!g_attr_set[MODE]) {
+  const int dev = current_device();
+  if (dev < 0) return MOE_ERR_CUDA;
+  if (!g_attr_set[dev][MODE]) {
     MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    g_attr_set[MODE] = true;
+    g_attr_set[dev][MODE] = true;
   }
-  if (g_sm_count == 0) {
-    int dev = 0;
-    MOE_CUDA(cudaGetDevice(&dev));
-    MOE_CUDA(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
-  }
-  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(g_sm_count, max_tiles));
+  const int sms = device_sm_count();
+  if (sms <= 0) return MOE_ERR_CUDA;
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_tiles));
   MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, p);
   return MOE_OK;
 }

@@ -225,7 +225,7 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
                                  const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
                                  void* stream) {
   if (!cfg || !X || !Wr || !Y || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(validate(cfg));
+  MOE_CHECK(layer_preflight(cfg, false));
   if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
   const bool shared = cfg->F_shared > 0;
   const bool fp8 = cfg->dtype == 2;
@@ -311,7 +311,7 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
                                  const void* Wd_s, const void* ctx, void* dX, void* dWr, void* dWg, void* dWu,
                                  void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, void* ws, void* stream) {
   if (!cfg || !dY || !X || !Wr || !ctx || !dX || !ws) return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(validate(cfg));
+  MOE_CHECK(layer_preflight(cfg, true));
   const bool shared = cfg->F_shared > 0;
   const bool fp8 = cfg->dtype == 2;   // fp8: the dgrad reads the codes saved in ctx; the bf16 weights are not touched
   if (!fp8 && (!Wg || !Wu || !Wd)) return MOE_ERR_INVALID_ARG;
@@ -407,7 +407,12 @@ extern "C" int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const
                                    void* dWg, void* dWu, void* dWd, void* dWg_s, void* dWu_s, void* dWd_s,
                                    int32_t accumulate_fp32, void* stream) {
   if (!cfg || !X || !dY || !ctx || !ws || !dWg || !dWu || !dWd) return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(validate(cfg));
+  MOE_CHECK(layer_preflight(cfg, true));
+  {   // the fp32-accumulate and fp8 weight gradients exist on the tensor-core path only: say so before any launch
+    const bool tc_ok = cfg->dtype != 0 && cfg->H % 64 == 0 && cfg->F % 64 == 0 && cfg->row_align % 128 == 0 &&
+                       (cfg->F_shared % 64 == 0);
+    if ((accumulate_fp32 || cfg->dtype == 2) && !tc_ok) return MOE_ERR_UNSUPPORTED;
+  }
   const bool shared = cfg->F_shared > 0;
   const bool wgrad_s = dWg_s || dWu_s || dWd_s;
   if (wgrad_s && !(shared && dWg_s && dWu_s && dWd_s)) return MOE_ERR_INVALID_ARG;

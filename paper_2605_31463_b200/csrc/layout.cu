@@ -24,6 +24,27 @@ int32_t validate(const moe_config_t* c) {
   return MOE_OK;
 }
 
+int32_t layer_preflight(const moe_config_t* c, bool backward) {
+  MOE_CHECK(validate(c));
+  // moe_route (route.cu): one warp per token holds E/32 keys per lane, K <= 32 output slots, one lane per group
+  if (c->E > 1024 || c->K > 32 || c->n_group > 32) return MOE_ERR_UNSUPPORTED;
+  // fp8 expert GEMMs need 128-row tiles that belong to one expert
+  if (c->dtype == 2 && c->row_align % 128 != 0) return MOE_ERR_UNSUPPORTED;
+  (void)backward;
+  return MOE_OK;
+}
+
+int device_sm_count() {
+  static int sm[MAX_DEVICES] = {0};
+  const int d = current_device();
+  if (d < 0) return 0;
+  if (sm[d] == 0 && cudaDeviceGetAttribute(&sm[d], cudaDevAttrMultiProcessorCount, d) != cudaSuccess) {
+    cudaGetLastError();
+    sm[d] = 0;
+  }
+  return sm[d];
+}
+
 namespace {
 struct Carver {
   size_t cur = 0;
@@ -188,13 +209,21 @@ namespace {
 constexpr int MAX_MARKS = 8192;
 cudaEvent_t g_ev[MAX_MARKS];
 int g_ev_stage[MAX_MARKS];
-int g_ev_created = 0, g_ev_used = 0;
+int g_ev_created = 0, g_ev_used = 0, g_ev_device = -1;
+bool g_ev_overflow = false;
 const char* const kStageNames[ST_COUNT] = {"begin", "router_gemm", "route", "maps", "permute", "gemm1_swiglu", "gemm2",
                                            "combine", "combine_bwd", "dgrad_down_swiglu", "dgrad_gateup", "wgrad",
                                            "router_bwd", "dx_combine", "shared_fwd", "shared_bwd", "quant"};
 }  // namespace
 void prof_mark_impl(int stage, cudaStream_t s) {
-  if (g_ev_used >= MAX_MARKS) return;
+  if (g_ev_used >= MAX_MARKS) { g_ev_overflow = true; return; }   // reported by moe_profile_stage_ms, never silently dropped
+  const int dev = current_device();
+  if (dev != g_ev_device) {            // events belong to the device they were created on: start over on a new one
+    for (int i = 0; i < g_ev_created; ++i) cudaEventDestroy(g_ev[i]);
+    cudaGetLastError();
+    g_ev_created = g_ev_used = 0;
+    g_ev_device = dev;
+  }
   if (g_ev_used >= g_ev_created) {
     if (cudaEventCreate(&g_ev[g_ev_created]) != cudaSuccess) { cudaGetLastError(); return; }
     ++g_ev_created;
@@ -207,6 +236,7 @@ void prof_mark_impl(int stage, cudaStream_t s) {
 extern "C" int32_t moe_profile_enable(int32_t on) {
   g_prof_on = on ? 1 : 0;
   g_ev_used = 0;
+  g_ev_overflow = false;
   return MOE_OK;
 }
 
@@ -216,6 +246,7 @@ extern "C" int32_t moe_profile_stage_ms(const char* stage, double* total_ms, int
   for (int i = 1; i < ST_COUNT; ++i)
     if (strcmp(kStageNames[i], stage) == 0) want = i;
   if (want < 0) return MOE_ERR_INVALID_ARG;
+  if (g_ev_overflow) return MOE_ERR_WORKSPACE;   // more than MAX_MARKS marks since moe_profile_enable: totals would be truncated
   double sum = 0;
   int64_t n = 0;
   for (int i = 1; i < g_ev_used; ++i) {

@@ -67,3 +67,32 @@ def test_invalid_configs_are_rejected_on_the_host(moe):
     # NULL pointers: INVALID_ARG before anything is enqueued (no CUDA call happens)
     st = moe.lib().moe_route(C.byref(moe.make_config(wl.TINY)), None, None, None, None, None)
     assert st == moe.MOE_ERR_INVALID_ARG
+
+
+def test_pipeline_object_is_validated_on_the_host(moe):
+    """moe_layer_step_host_pipelined keeps its ordering events in a caller-owned object: a NULL / dead handle is
+    INVALID_ARG before anything is enqueued; creating one needs a CUDA device (MOE_ERR_CUDA here)."""
+    l = moe.lib()
+    assert l.moe_pipeline_destroy(None) == moe.MOE_ERR_INVALID_ARG
+    args = [None] * 30
+    st = l.moe_layer_step_host_pipelined(None, C.byref(moe.make_config(wl.TINY)), 0, *args)
+    assert st == moe.MOE_ERR_INVALID_ARG
+    import torch
+    if not torch.cuda.is_available():
+        h = C.c_void_p(None)
+        assert l.moe_pipeline_create(C.byref(h)) == moe.MOE_ERR_CUDA and not h.value
+
+
+def test_layer_calls_reject_unsupported_configs_before_any_launch(moe):
+    """UNSUPPORTED is decided by the pre-flight, not by the stage that would hit the limit: with dummy non-NULL
+    pointers and no GPU the call must return UNSUPPORTED (a launch attempt would return MOE_ERR_CUDA instead)."""
+    l = moe.lib()
+    bad = wl.QWEN3_SMALL.replace(E=2048, K=4)                      # moe_route holds at most 1024 experts per warp
+    dummy = C.c_void_p(256)
+    st = l.moe_layer_fwd(C.byref(moe.make_config(bad)), *([dummy] * 14), None)
+    assert st == moe.MOE_ERR_UNSUPPORTED
+    st = l.moe_layer_bwd(C.byref(moe.make_config(bad)), *([dummy] * 19), None)
+    assert st == moe.MOE_ERR_UNSUPPORTED
+    fp8_unaligned = wl.DSV3_FP8_SMALL.replace(row_align=1)
+    st = l.moe_layer_fwd(C.byref(moe.make_config(fp8_unaligned)), *([dummy] * 14), None)
+    assert st == moe.MOE_ERR_UNSUPPORTED

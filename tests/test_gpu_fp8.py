@@ -127,19 +127,27 @@ def test_fp8_layer_fwd_bwd_matches_fake_quant_oracle(cfg):
     print(cfg.name, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
 
 
-def test_fp8_weight_cache_reuses_codes(env):
-    """moe_layer_fwd with NULL weights reuses the codes left in ctx (PAPER.md:116 FP8 weight cache)."""
+def test_fp8_weight_cache_matches_oracle(env):
+    """FP8 weight cache: quantise the weights once with moe_fp8_quantize_weights, then run a NEW
+    micro-batch through moe_layer_fwd with NULL weights (the bf16 weights overwritten with garbage first, so nothing
+    can read them) and moe_layer_bwd; every output is compared with the fake-quant ORACLE on that micro-batch."""
     torch, moe, buffers = env
     cfg = wl.DSV3_FP8_SMALL.replace(row_align=128)
     inp = gc.gen_inputs(cfg)
-    lb = gc.run_gpu_layer(cfg, inp)
-    Y0, dX0 = lb.Y.clone(), lb.dX.clone()
-    lb.Y.zero_(); lb.dX.zero_()
+    lb = buffers.LayerBuffers(cfg)
+    lb.load(**inp)
+    moe.moe_fp8_quantize_weights(lb.ccfg, lb.Wg, lb.Wu, lb.Wd, lb.Wg_s, lb.Wu_s, lb.Wd_s, lb.ctx)
+    inp2 = dict(inp, X=wl.gen_X(cfg.replace(seed=9)), dY=wl.gen_dY(cfg.replace(seed=9)))
+    lb.load(X=inp2["X"], dY=inp2["dY"])
+    for w in (lb.Wg, lb.Wu, lb.Wd, lb.Wg_s, lb.Wu_s, lb.Wd_s):
+        w.fill_(float("nan"))
     moe.moe_layer_fwd(lb.ccfg, lb.X, lb.Wr, lb.bias, None, None, None, None, None, None, lb.Y, lb.topk_idx, lb.topk_w,
                       lb.ctx, lb.ws)
-    lb.backward()
+    moe.moe_layer_bwd(lb.ccfg, lb.dY, lb.X, lb.Wr, None, None, None, None, None, None, lb.ctx, lb.dX, lb.dWr, lb.dWg,
+                      lb.dWu, lb.dWd, lb.dWg_s, lb.dWu_s, lb.dWd_s, lb.ws)
     torch.cuda.synchronize()
-    assert torch.equal(lb.Y, Y0) and torch.equal(lb.dX, dX0)
+    errs = gc.compare_layer(cfg, inp2, lb)
+    print(cfg.name, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
 
 
 def test_fp8_rejects_unaligned():

@@ -119,8 +119,9 @@ def test_full_size_sampled_outputs(cfg0):
     shared = None
     if cfg.F_shared:
         shared = tuple(to_numpy(t) for t in (lb.Wg_s, lb.Wu_s, lb.Wd_s))
-    tokens = [T // 3] if fp8 else [0, T // 3, T - 1]     # fp8: each expert costs the oracle ~5 s of fake-quantisation
+    tokens = [0, T // 3, T - 1]
     Y_g, dX_g, dw_g = to_numpy(lb.Y), to_numpy(lb.dX), to_numpy(lb.ws_view("dw"))
+    dz_g = to_numpy(lb.ws_view("dz")).astype(np.float64)                  # [T, K]: dz of the selected experts
     Wr64 = Wr.astype(np.float64)
     for t in tokens:
         Yt = np.zeros(H); dXt = np.zeros(H); dwt = np.zeros(K)
@@ -141,6 +142,7 @@ def test_full_size_sampled_outputs(cfg0):
                 dXp = orc.expert_ffn_bwd(dy, X64[t:t + 1], g, u, a, *W3)[0]
             dXt += dXp[0]
         dz = orc.router_bwd(cfg.replace(T=1), z_o[t:t + 1], idx[t:t + 1], w64[t:t + 1], dwt[None, :])
+        note("dz", orc.rel_fro(dz_g[t], dz[0, idx[t].astype(np.int64)]))   # router-bwd rows of the sampled tokens
         dXt += (dz @ Wr64)[0]
         if shared is not None:
             g, u, a, y = ffn_fwd(Xq[t:t + 1], shared)
@@ -150,6 +152,34 @@ def test_full_size_sampled_outputs(cfg0):
             else:
                 dXt += orc.expert_ffn_bwd(dY64[t:t + 1], X64[t:t + 1], g, u, a, *shared)[0][0]
         note("Y", orc.rel_fro(Y_g[t], Yt)); note("dX", orc.rel_fro(dX_g[t], dXt)); note("dw", orc.rel_fro(dw_g[t], dwt))
+    # ---- dWr, stage-wise (replay style): the GPU's dz rows (verified above on the sampled tokens against
+    # oracle.router_bwd) scattered to [T, E] and contracted with X in fp64: dWr[e] = sum_t dz[t, e] X[t], all experts ----
+    dz_dense = np.zeros((T, E))
+    np.put_along_axis(dz_dense, idx.astype(np.int64), dz_g, axis=1)
+    dWr_ref = dz_dense.T @ X64
+    dWr_g = to_numpy(lb.dWr)
+    for e in range(E):
+        if counts[e]:
+            note("dWr", orc.rel_fro(dWr_g[e], dWr_ref[e]))
+        else:
+            assert not dWr_g[e].any(), "an expert no token selected has dWr == 0 exactly"
+
+    # ---- shared expert (single-group path, T-row contractions): a 256-column slab of dWg_s / dWu_s (rows of the
+    # [F_s, H] gradients) and of dWd_s (columns of [H, F_s]) against the oracle's single-expert backward ----
+    if shared is not None:
+        Fs = cfg.F_shared
+        f0 = (Fs // 2) // 128 * 128
+        sl = slice(f0, f0 + 256)
+        W3 = (shared[0][sl], shared[1][sl], np.ascontiguousarray(shared[2][:, sl]))   # [256,H], [256,H], [H,256]
+        g, u, a, _ = ffn_fwd(Xq, W3)
+        if fp8:
+            _, dWg, dWu, dWd, _, _ = orc.expert_ffn_bwd_fp8(dYq, np.ones(T), dY64, X64, g, u, a, *W3, mode)
+        else:
+            _, dWg, dWu, dWd, _, _ = orc.expert_ffn_bwd(dY64, X64, g, u, a, *W3)
+        note("dWg_s", orc.rel_fro(to_numpy(lb.dWg_s[sl]), dWg)); note("dWu_s", orc.rel_fro(to_numpy(lb.dWu_s[sl]), dWu))
+        note("dWd_s", orc.rel_fro(to_numpy(lb.dWd_s[:, sl]), dWd))
+        gu_s = lb.ctx_view("gu_s")
+        note("g_s", orc.rel_fro(to_numpy(gu_s[:, sl]), g)); note("u_s", orc.rel_fro(to_numpy(gu_s[:, Fs + f0:Fs + f0 + 256]), u))
     print(cfg.name, {k: f"{v:.2e}" for k, v in worst.items()})
     bad = {k: v for k, v in worst.items() if not v <= tol}
     assert not bad, f"{cfg.name}: over tolerance {tol}: {bad}; all {worst}"

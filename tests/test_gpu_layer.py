@@ -105,9 +105,11 @@ WGRAD_CASES = [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128
 
 @pytest.mark.parametrize("cfg", WGRAD_CASES, ids=lambda c: c.name)
 def test_delayed_wgrad_overwrite_and_fp32_accumulate(cfg):
-    """moe_layer_wgrad after a dgrad-only backward (PAPER.md:116 wgrad delay): (a) bf16 overwrite reproduces the fused
-    backward bit for bit; (b) fp32 accumulation adds the gradient to what the buffers held (two calls add it twice;
-    an empty expert's slice is untouched)."""
+    """moe_layer_wgrad after a dgrad-only backward (PAPER.md:116 wgrad delay): (a) bf16 overwrite equals the fused
+    backward bit for bit AND the oracle (the fused backward's gradients are oracle-checked in
+    test_layer_fwd_bwd_matches_oracle; here dX and the delayed gradients are compared with the oracle again);
+    (b) fp32 accumulation adds the gradient to what the buffers held: two calls add it twice, the sum is compared
+    with the fp64 oracle at a tighter tolerance than bf16 outputs allow, an empty expert's slice is untouched."""
     import torch
     import paper_2605_31463_b200 as moe
     from paper_2605_31463_b200.buffers import LayerBuffers, to_numpy
@@ -124,6 +126,15 @@ def test_delayed_wgrad_overwrite_and_fp32_accumulate(cfg):
     assert torch.equal(lb.dX, full.dX)
     for n in names:
         assert torch.equal(out[n], getattr(full, n)), n
+    gc.compare_layer(cfg, inp, full)                                       # ... and the fused backward equals the oracle
+    # (b) fp32 main gradients: compared with the ORACLE.  fp32 accumulation removes the bf16 rounding of the output, what is
+    # left is the rounding of the bf16 operands (dy, a, dg, du: 2^-9/sqrt(3) ~ 1e-3 relative each, not averaged away
+    # by a random-sign contraction), so the bound is 3e-3 (bf16 outputs: 1e-2); FP8 keeps its own tolerance because the
+    # dgrad feeding dg, du is quantised.
+    tol32 = 3e-3 if cfg.dtype == wl.DTYPE_BF16 else gc.TOL[cfg.dtype]
+    idx_gpu = to_numpy(lb.topk_idx)
+    fwd_o = orc.layer_fwd(cfg, inp["X"], inp["Wr"], inp["bias"], inp["W"], inp["shared"], forced_idx=idx_gpu)
+    bwd_o = orc.layer_bwd(cfg, inp["dY"], inp["X"], inp["Wr"], inp["W"], fwd_o, inp["shared"])
     g0 = {n: torch.randn(getattr(full, n).shape, device="cuda", dtype=torch.float32) for n in names}
     acc = {n: g0[n].clone() for n in names}
     args = [acc.get(n) for n in ("dWg", "dWu", "dWd", "dWg_s", "dWu_s", "dWd_s")]
@@ -131,17 +142,21 @@ def test_delayed_wgrad_overwrite_and_fp32_accumulate(cfg):
     moe.moe_layer_wgrad(lb.ccfg, lb.X, lb.dY, lb.ctx, lb.ws, *args, 1)
     torch.cuda.synchronize()
     counts = to_numpy(lb.ctx_view("counts"))
+    worst = 0.0
     for n in names:
-        added = (acc[n] - g0[n]).double().cpu().numpy()
-        ref = 2.0 * to_numpy(getattr(full, n)).astype(np.float64)          # the bf16 gradient, itself oracle-checked
+        added = (acc[n].double() - g0[n].double()).cpu().numpy()
+        ref = 2.0 * bwd_o[n]                                               # two micro-batches of the same gradient
         if added.ndim == 3:
             for e in range(cfg.E):
                 if counts[e] == 0:
                     assert torch.equal(acc[n][e], g0[n][e]), (n, e)
                 else:
-                    assert orc.rel_fro(added[e], ref[e]) <= 1e-2, (n, e, orc.rel_fro(added[e], ref[e]))
+                    err = orc.rel_fro(added[e], ref[e]); worst = max(worst, err)
+                    assert err <= tol32, (n, e, err)
         else:
-            assert orc.rel_fro(added, ref) <= 1e-2, n
+            err = orc.rel_fro(added, ref); worst = max(worst, err)
+            assert err <= tol32, (n, err)
+    print(cfg.name, f"fp32-accumulated wgrad vs oracle: worst {worst:.2e} (tol {tol32})")
 
 
 def test_pipelined_host_step_matches_device_step():

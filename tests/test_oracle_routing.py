@@ -89,6 +89,28 @@ def test_bias_is_selection_only():
     assert np.abs(w[:, 0] - c.routed_scale * s5 / ssum).max() < 1e-14       # the bias is not in w
 
 
+def test_zipf_offset_is_a_selection_offset_on_the_softmax_path():
+    """configs[4] reading (S21): the Zipf per-expert offset o[e] skews WHICH experts are chosen
+    (key = z + o) while the gating weights are the softmax over the chosen experts' UNBIASED logits.
+    Selection is pinned by brute force on z + o, the weights by torch.softmax on the gathered z, and the
+    load skew (top 5 % of experts ~ 40 % of the rows, empty experts exist) by counting."""
+    import torch
+    c = wl.GPTOSS_SMALL
+    z = wl.gen_logits(c).astype(np.float64)
+    o = wl.gen_bias(c)
+    idx, w = O.route(z, o, c)
+    assert np.array_equal(idx, brute_topk(z + o.astype(np.float64)[None, :], c.K))
+    zs = torch.from_numpy(np.take_along_axis(z, idx.astype(np.int64), axis=1))
+    assert np.abs(w - torch.softmax(zs, dim=1).numpy()).max() < 1e-15
+    w_biased = torch.softmax(zs + torch.from_numpy(o.astype(np.float64))[torch.from_numpy(idx.astype(np.int64))], dim=1).numpy()
+    assert np.abs(w - w_biased).max() > 1e-2                                # the two readings really differ
+    cfull = wl.GPTOSS
+    counts = np.bincount(O.route(wl.gen_logits(cfull).astype(np.float64), wl.gen_bias(cfull), cfull)[0].reshape(-1),
+                         minlength=cfull.E)
+    top = np.sort(counts)[::-1]
+    assert 0.35 < top[:6].sum() / counts.sum() < 0.55 and (counts == 0).sum() >= 4
+
+
 def test_group_limit_reductions_and_membership():
     c = wl.DSV3_SMALL
     z = wl.gen_logits(c).astype(np.float64)
