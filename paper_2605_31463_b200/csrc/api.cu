@@ -4,6 +4,7 @@
 
 #include "fp8.cuh"
 #include "gemm_tc.cuh"
+#include "tile_tables.cuh"
 
 using namespace moe;
 
@@ -31,6 +32,7 @@ extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int3
     TcCall c;
     memset(&c, 0, sizeof(c));
     c.mode = TC_FWD; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    c.plist = mtile + tile_plist_off(c.rows_cap); c.olist = mtile + tile_olist_off(c.rows_cap);
     c.A = A; c.lda = Kdim; c.B0 = B; c.b_rows = N; c.b_cols = Kdim; c.N = N; c.Kd = Kdim; c.out0 = C; c.ld0 = N;
     const int32_t st = tc_gemm(c, s);
     if (st != MOE_ERR_UNSUPPORTED) return st;
@@ -53,6 +55,7 @@ extern "C" int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int3
     TcCall c;
     memset(&c, 0, sizeof(c));
     c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    c.plist = mtile + tile_plist_off(c.rows_cap); c.olist = mtile + tile_olist_off(c.rows_cap);
     if (dA) {   // dA = dC B[e]: contraction over B's rows
       c.mode = TC_DGRAD; c.A = dC; c.lda = N; c.B0 = B; c.B1 = nullptr; c.b_rows = N; c.b_cols = Kdim; c.N = Kdim;
       c.out0 = dA; c.ld0 = Kdim;

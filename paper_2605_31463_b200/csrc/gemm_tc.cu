@@ -11,12 +11,14 @@
 // Both K-major and MN-major shared-memory operand layouts are used, so the dgrad (weights read
 // "transposed") and wgrad (both operands contracted over rows) need no transposed copies in HBM.
 #include <cuda.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
 
 #include "gemm_tc.cuh"
 #include "tc_ptx.cuh"
+#include "tile_tables.cuh"
 
 namespace moe {
 
@@ -80,13 +82,25 @@ constexpr int BM = 128;      // tile rows  (UMMA M)
 constexpr int BN = 256;      // tile cols  (UMMA N)
 constexpr int BK = 64;       // k-block: 64 bf16 = 128 bytes = one swizzle span
 constexpr int UK = 16;       // UMMA K for 16-bit operands
-constexpr int STAGES = 4;
-constexpr int A_BYTES = BM * BK * 2;   // 16 KB
-constexpr int B_BYTES = BN * BK * 2;   // 32 KB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int A_BYTES = BM * BK * 2;   // 16 KB: this CTA's 128 rows of the left operand
+constexpr int B_BYTES = BN * BK * 2;   // 32 KB: all 256 columns of the right operand (a CTA of a pair holds half)
+// Per-CTA operand ring.  1-CTA kernel: 4 stages of (A 16 KB + B 32 KB).  CTA-pair kernel (cta_group::2, M = 256): each
+// CTA stages its own 128 A rows and HALF of B (the pair's tensor cores read both halves), 5 stages of 32 KB, so a
+// k-block costs each SM 32 KB of L2 -> SM traffic instead of 48 KB for the same 128 x 256 x 64 MACs; the 32 KB this
+// saves hold a second staging box per epilogue warp group (NOBUF), so a group fills one box while the TMA store of
+// its other box is still reading shared memory.
+template <bool PAIR> struct Ring {
+  static constexpr int STAGES = PAIR ? 5 : 4;
+  static constexpr int B_CTA = PAIR ? B_BYTES / 2 : B_BYTES;
+  static constexpr int STAGE_BYTES = A_BYTES + B_CTA;
+  static constexpr int NOBUF = PAIR ? 2 : 1;   // staging boxes per epilogue warp group
+};
+constexpr int MAX_STAGES = 6;
 constexpr int MN_BOX_BYTES = 64 * BK * 2;  // one 64(MN) x 64(K) box of an MN-major operand: 8 KB
 constexpr int OBUF_BYTES = BM * 128;       // epilogue staging: 128 rows x 64 bf16 columns (one 128-byte-swizzled TMA box)
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 2 * OBUF_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int SMEM_BYTES = Ring<false>::STAGES * Ring<false>::STAGE_BYTES + 2 * OBUF_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+static_assert(Ring<true>::STAGES * Ring<true>::STAGE_BYTES + 2 * Ring<true>::NOBUF * OBUF_BYTES ==
+              Ring<false>::STAGES * Ring<false>::STAGE_BYTES + 2 * Ring<false>::NOBUF * OBUF_BYTES, "same shared-memory footprint");
 constexpr int EPI_WARPS = 8;            // two per TMEM lane group: column-chunk parity `ch` splits a tile between them
 constexpr int NTHREADS = 64 + EPI_WARPS * 32;
 constexpr int TMEM_COLS = 512;
@@ -97,8 +111,10 @@ constexpr int TMEM_COLS = 512;
 struct TcParams {
   int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, tma_out, acc_f32;
   int64_t rows_valid;
-  const int32_t* mtile;
+  const int32_t* mtile;    // M-tile -> expert (nullptr: one group of rows_valid rows)
+  const int32_t* tlist;    // which M-tiles this launch runs: pair kernel = plist, 1-CTA kernel = olist or nullptr (all)
   const int32_t* offsets;
+  const int32_t* counts;   // WGRAD: real rows per expert (nullptr: contract over the whole 128-aligned group)
   __nv_bfloat16* out0;
   int64_t ld0;
   __nv_bfloat16* out1;
@@ -111,27 +127,31 @@ struct Tile {
   int e, m0, n0, nkb, row0;
 };
 
-template <int MODE>
-__device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_t total, Tile& tl) {
+// Tile t of this launch for the CTA of pair-rank `rank` (0 in the 1-CTA kernel).  A pair works on two consecutive
+// M-tiles of one expert (rows m0 = first tile + 128 rank) and the same 256 output columns.
+template <int MODE, bool PAIR>
+__device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_t total, int rank, Tile& tl) {
   if (t >= total) return false;
   if (MODE == TC_WGRAD) {
     const int per_e = p.m_tiles * p.n_tiles;
     tl.e = (int)(t / per_e);
     const int r = (int)(t - (int64_t)tl.e * per_e);
-    tl.m0 = (r / p.n_tiles) * BM;
+    tl.m0 = (r / p.n_tiles) * (PAIR ? 2 * BM : BM) + rank * BM;
     tl.n0 = (r % p.n_tiles) * BN;
     if (p.mtile) {
+      // k-blocks of 64 rows up to the expert's last real row: the 128-row alignment padding (zero rows) is skipped
       tl.row0 = p.offsets[tl.e];
-      tl.nkb = (p.offsets[tl.e + 1] - tl.row0) / BK;
+      tl.nkb = p.counts ? (p.counts[tl.e] + BK - 1) / BK : (p.offsets[tl.e + 1] - tl.row0) / BK;
     } else {
       tl.row0 = 0;
       tl.nkb = (int)((p.rows_valid + BK - 1) / BK);
     }
   } else {
-    // n fastest: consecutive CTAs share the 128-row activation tile
-    const int mt = (int)(t / p.n_tiles);
-    tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
-    tl.m0 = mt * BM;
+    // n fastest: consecutive CTAs / pairs share the activation rows
+    const int mi = (int)(t / p.n_tiles);
+    tl.n0 = (int)(t - (int64_t)mi * p.n_tiles) * (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);
+    const int mt = p.tlist ? p.tlist[1 + mi] : (PAIR ? 2 * mi : mi);
+    tl.m0 = (mt + rank) * BM;
     tl.e = p.mtile ? p.mtile[1 + mt] : 0;
     tl.nkb = p.nkb;
     tl.row0 = 0;
@@ -139,10 +159,13 @@ __device__ __forceinline__ bool decode_tile(const TcParams& p, int64_t t, int64_
   return true;
 }
 
-template <int MODE>
+template <int MODE, bool PAIR>
 __device__ __forceinline__ int64_t total_tiles(const TcParams& p) {
   if (MODE == TC_WGRAD) return (int64_t)p.E * p.m_tiles * p.n_tiles;
-  const int64_t mt = p.mtile ? p.mtile[0] : (p.rows_valid + BM - 1) / BM;
+  int64_t mt;
+  if (p.tlist) mt = p.tlist[0];
+  else if (p.mtile) mt = PAIR ? 0 : p.mtile[0];
+  else mt = (p.rows_valid + (PAIR ? 2 * BM : BM) - 1) / (PAIR ? 2 * BM : BM);
   return mt * p.n_tiles;
 }
 
@@ -415,13 +438,16 @@ __device__ __forceinline__ void gu_tma_fetch(const TcParams& p, const Tile& tl, 
 // box (thread = row, conflict-free 16-byte stores) and written with one TMA store (full 128-byte lines; rows past M
 // and columns past N are clipped by the 3-D tensor map [E, M, N]).  The two column-parity warp groups own one box each
 // and alternate, so one group's TMA store overlaps the other group's TMEM drain.
+// `rel` = what releases the accumulator (called by every thread right after the tile's last TMEM load, before the
+// last chunk is staged); `seq` = running chunk counter of this warp group, selecting which of its NB staging boxes
+// a chunk uses.
+template <int NB, typename Rel>
 __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
-                                                 bool have_acc, uint32_t obuf, const CUtensorMap* tmO, bool issuer,
-                                                 int ch, int ecoord) {
+                                                 bool have_acc, uint32_t obuf0g, const CUtensorMap* tmO, bool issuer,
+                                                 int ch, int ecoord, uint32_t& seq, Rel rel) {
+  const int nch = min(BN / 64, (p.N - tl.n0 + 63) / 64);   // 64-column chunks of this tile inside N (warp-uniform)
 #pragma unroll 1
-  for (int c = ch; c < BN / 64; c += 2) {
-    const int ncols = p.N - (tl.n0 + c * 64);   // warp-uniform
-    if (ncols <= 0) break;
+  for (int c = ch; c < nch; c += 2) {
     uint32_t v0[32], v1[32];
     if (have_acc) {
       tmem_ld32(tacc + c * 64, v0);
@@ -431,7 +457,13 @@ __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& 
 #pragma unroll
       for (int i = 0; i < 32; ++i) v0[i] = v1[i] = 0u;   // empty expert: exact zeros
     }
-    if (issuer) bulk_wait_read0();     // this group's previous TMA store has finished reading the box
+    if (c + 2 >= nch) rel();           // accumulator drained: the next tile's MMAs may overwrite it
+    const uint32_t obuf = obuf0g + (NB == 2 ? (seq & 1u) * OBUF_BYTES : 0u);
+    ++seq;
+    if (issuer) {                      // the TMA store that last used this box has finished reading it
+      if (NB == 2) bulk_wait_read1();
+      else bulk_wait_read0();
+    }
     named_bar_sync(1 + ch, 128);
     const uint32_t rowaddr = obuf + row_in_tile * 128;
     const int sw = row_in_tile & 7;
@@ -453,21 +485,29 @@ __device__ __forceinline__ void wgrad_store_tile(const TcParams& p, const Tile& 
       bulk_commit();
     }
   }
+  if (ch >= nch) rel();                // this warp group has no chunk in the tile (N tail): still one release per warp
 }
 
 // TC_WGRAD with fp32 accumulation into an existing gradient (dB += tile; PAPER.md:116 wgrad delay keeps fp32 main
 // gradients across micro-batches): 32-column fp32 chunks (128-byte rows) staged like above and added by a TMA
 // reduce-add store, so the old gradient is never read by the SM.  An empty expert adds nothing.
+template <int NB, typename Rel>
 __device__ __forceinline__ void wgrad_accum_tile(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
-                                                 uint32_t obuf, const CUtensorMap* tmO, bool issuer, int ch) {
+                                                 uint32_t obuf0g, const CUtensorMap* tmO, bool issuer, int ch, uint32_t& seq,
+                                                 Rel rel) {
+  const int nch = min(BN / 32, (p.N - tl.n0 + 31) / 32);
 #pragma unroll 1
-  for (int c = ch; c < BN / 32; c += 2) {
-    const int ncols = p.N - (tl.n0 + c * 32);   // warp-uniform
-    if (ncols <= 0) break;
+  for (int c = ch; c < nch; c += 2) {
     uint32_t v[32];
     tmem_ld32(tacc + c * 32, v);
     tmem_ld_wait();
-    if (issuer) bulk_wait_read0();
+    if (c + 2 >= nch) rel();
+    const uint32_t obuf = obuf0g + (NB == 2 ? (seq & 1u) * OBUF_BYTES : 0u);
+    ++seq;
+    if (issuer) {
+      if (NB == 2) bulk_wait_read1();
+      else bulk_wait_read0();
+    }
     named_bar_sync(1 + ch, 128);
     const uint32_t rowaddr = obuf + row_in_tile * 128;
     const int sw = row_in_tile & 7;
@@ -480,27 +520,38 @@ __device__ __forceinline__ void wgrad_accum_tile(const TcParams& p, const Tile& 
       bulk_commit();
     }
   }
+  if (ch >= nch) rel();
 }
 
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <int MODE>
+// PAIR = false: one CTA per SM, tcgen05 cta_group::1, 128 x 256 tiles (the unpaired M-tiles, see tile_tables.cuh).
+// PAIR = true : launched as clusters of two CTAs (one TPC).  The pair computes a 256 x 256 tile with cta_group::2 MMAs
+//   issued by the leader (rank 0): each CTA stages its own 128 rows of A and one half of B; TMA bytes of both CTAs are
+//   signalled on the leader's full barrier; tcgen05.commit multicasts "stage free" / "accumulator ready" to both CTAs;
+//   each CTA's epilogue warps drain their own 128 TMEM lanes and release the accumulator on the leader's barrier.
+template <int MODE, bool PAIR>
 __global__ void __launch_bounds__(NTHREADS, 1)
 tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
                const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmO,
                const __grid_constant__ CUtensorMap tmO2, const TcParams p) {
   constexpr bool A_MN = (MODE == TC_WGRAD);
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
+  constexpr int STAGES = Ring<PAIR>::STAGES, STAGE_BYTES = Ring<PAIR>::STAGE_BYTES, B_CTA = Ring<PAIR>::B_CTA;
+  constexpr int NOBUF = Ring<PAIR>::NOBUF, GROUP_OBUF = NOBUF * OBUF_BYTES;   // staging bytes of one epilogue warp group
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128-byte swizzle wants 1024-byte alignment
   const uint32_t obuf0 = base + STAGES * STAGE_BYTES;
-  const uint32_t bars = obuf0 + 2 * OBUF_BYTES;
-  // barrier addresses: full[s] = bars + 8 s; empty[s] = bars + 8 (STAGES + s); tfull[a] / tempty[a] follow
-  const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull0 = bars + 16 * STAGES, tempty0 = tfull0 + 16;
+  const uint32_t bars = obuf0 + 2 * GROUP_OBUF;
+  // barrier addresses: full[s] = bars + 8 s; empty[s] = bars + 8 (MAX_STAGES + s); tfull[a] / tempty[a] follow
+  const uint32_t full0 = bars, empty0 = bars + 8 * MAX_STAGES, tfull0 = bars + 16 * MAX_STAGES, tempty0 = tfull0 + 16;
   const uint32_t tmem_slot = tempty0 + 16;
   const uint32_t gbar0 = tempty0 + 24;   // two barriers: g, u boxes of the dgrad-down epilogue groups
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = PAIR ? (int)cluster_ctarank() : 0;              // 0 = pair leader (issues the MMAs)
+  const int64_t unit = PAIR ? (blockIdx.x >> 1) : blockIdx.x;      // index of this CTA / pair among the launch's workers
+  const int64_t nunits = PAIR ? (gridDim.x >> 1) : gridDim.x;
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmA);
@@ -514,67 +565,91 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull0 + 8 * a, 1);
-      mbar_init(tempty0 + 8 * a, EPI_WARPS);   // one arrive per epilogue warp
+      mbar_init(tempty0 + 8 * a, PAIR ? 2 * EPI_WARPS : EPI_WARPS);   // one arrive per epilogue warp (of both CTAs)
       mbar_init(gbar0 + 8 * a, 1);
     }
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(tmem_slot, TMEM_COLS);
+  if (warp == 1) {
+    if (PAIR) tmem_alloc_pair(tmem_slot, TMEM_COLS);
+    else tmem_alloc(tmem_slot, TMEM_COLS);
+  }
   tc_fence_before();
-  __syncthreads();
+  __syncwarp();
+  if (PAIR) cluster_sync_all();   // the peer's barriers are initialised before anything is signalled on them
+  else __syncthreads();
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  const int64_t total = total_tiles<MODE>(p);
+  const int64_t total = total_tiles<MODE, PAIR>(p);
 
   if (warp == 0) {
-    // ===================== TMA producer (one thread) =====================
+    // ===================== TMA producer (one thread per CTA) =====================
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      Tile tl;
-      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      // the next tile's schedule entry (two dependent global loads) is fetched while this tile's k-loop runs
+      Tile tl, nx;
+      bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+      for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
+        okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
+        const int bn0 = tl.n0 + (PAIR ? rank * (BN / 2) : 0);   // first of the B columns this CTA stages
         for (int kb = 0; kb < tl.nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, phase ^ 1);
-          const uint32_t fb = full0 + 8 * stage;
           const uint32_t sa = base + stage * STAGE_BYTES, sb = sa + A_BYTES;
-          mbar_expect_tx(fb, STAGE_BYTES);
+          uint32_t fb = full0 + 8 * stage;
+          if (PAIR) {
+            if (rank == 0) mbar_expect_tx(fb, 2 * STAGE_BYTES);   // both CTAs' boxes complete on the leader's barrier
+            fb = mapa_shared(fb, 0);
+          } else {
+            mbar_expect_tx(fb, STAGE_BYTES);
+          }
+          auto load = [&](uint32_t dst, const CUtensorMap* m, int c0, int c1) {
+            if (PAIR) tma_load_2d_pair(dst, m, fb, c0, c1);
+            else tma_load_2d(dst, m, fb, c0, c1);
+          };
           if (!A_MN) {
-            tma_load_2d(sa, &tmA, fb, kb * BK, tl.m0);                              // box 64 x 128
+            load(sa, &tmA, kb * BK, tl.m0);                                        // box 64 x 128
           } else {
             const int kr = tl.row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BM / 64; ++i) tma_load_2d(sa + i * MN_BOX_BYTES, &tmA, fb, p.a_col0 + tl.m0 + 64 * i, kr);
+            for (int i = 0; i < BM / 64; ++i) load(sa + i * MN_BOX_BYTES, &tmA, p.a_col0 + tl.m0 + 64 * i, kr);
           }
           if (MODE == TC_FWD || MODE == TC_FWD_F32) {
-            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 256
+            load(sb, &tmB0, kb * BK, tl.e * p.b_rows + bn0);                       // box 64 x 256 (pair: 64 x 128)
           } else if (MODE == TC_FWD_SWIGLU) {
-            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);            // box 64 x 128 (Wg)
-            tma_load_2d(sb + B_BYTES / 2, &tmB1, fb, kb * BK, tl.e * p.b_rows + tl.n0);  // (Wu)
+            if (PAIR) {                                                             // leader stages Wg, its peer Wu
+              load(sb, rank == 0 ? &tmB0 : &tmB1, kb * BK, tl.e * p.b_rows + tl.n0);
+            } else {
+              load(sb, &tmB0, kb * BK, tl.e * p.b_rows + tl.n0);                   // box 64 x 128 (Wg)
+              load(sb + B_BYTES / 2, &tmB1, kb * BK, tl.e * p.b_rows + tl.n0);     // (Wu)
+            }
           } else if (MODE == TC_WGRAD) {
             const int kr = tl.row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BN / 64; ++i) tma_load_2d(sb + i * MN_BOX_BYTES, &tmB0, fb, tl.n0 + 64 * i, kr);
+            for (int i = 0; i < B_CTA / MN_BOX_BYTES; ++i) load(sb + i * MN_BOX_BYTES, &tmB0, bn0 + 64 * i, kr);
           } else {
             const bool second = kb >= p.kb_split;
             const CUtensorMap* bm = second ? &tmB1 : &tmB0;
             const int kr = tl.e * p.b_rows + (second ? kb - p.kb_split : kb) * BK;
 #pragma unroll
-            for (int i = 0; i < BN / 64; ++i) tma_load_2d(sb + i * MN_BOX_BYTES, bm, fb, tl.n0 + 64 * i, kr);
+            for (int i = 0; i < B_CTA / MN_BOX_BYTES; ++i) load(sb + i * MN_BOX_BYTES, bm, bn0 + 64 * i, kr);
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread) =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = instr_desc(1, A_MN ? 1 : 0, B_MN ? 1 : 0, BN);
+    // ===================== MMA issuer (one thread; in a pair only the leader's) =====================
+    if (lane == 0 && rank == 0) {
+      constexpr uint32_t idesc = instr_desc(1, A_MN ? 1 : 0, B_MN ? 1 : 0, BN, PAIR ? 2 * BM : BM);
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
-      Tile tl;
-      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      Tile tl, nx;
+      bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+      for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
+        okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
         if (tl.nkb == 0) continue;
         mbar_wait(tempty0 + 8 * as, aphase ^ 1);
         tc_fence_after();
@@ -587,44 +662,49 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           for (int k = 0; k < BK / UK; ++k) {
             const uint64_t ad = A_MN ? smem_desc(sa + k * UK * 128, MN_BOX_BYTES, 1024) : smem_desc(sa + k * UK * 2, 16, 1024);
             const uint64_t bd = B_MN ? smem_desc(sb + k * UK * 128, MN_BOX_BYTES, 1024) : smem_desc(sb + k * UK * 2, 16, 1024);
-            umma_bf16(dacc, ad, bd, idesc, (kb | k) != 0);
+            if (PAIR) umma_bf16_pair(dacc, ad, bd, idesc, (kb | k) != 0);
+            else umma_bf16(dacc, ad, bd, idesc, (kb | k) != 0);
           }
-          umma_commit(empty0 + 8 * stage);   // frees the smem stage once these MMAs have read it
+          // frees the smem stage (in both CTAs of a pair) once these MMAs have read it
+          if (PAIR) umma_commit_pair(empty0 + 8 * stage);
+          else umma_commit(empty0 + 8 * stage);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        umma_commit(tfull0 + 8 * as);        // accumulator complete
+        if (PAIR) umma_commit_pair(tfull0 + 8 * as);   // accumulator complete
+        else umma_commit(tfull0 + 8 * as);
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
   } else {
-    // ===================== epilogue warps 2..5 =====================
+    // ===================== epilogue warps 2..9 =====================
     const int lg = warp & 3;                 // TMEM lane group this warp may access
     const int ch = (warp - 2) >> 2;          // which half of the column chunks this warp drains
     const int row_in_tile = lg * 32 + lane;
     int as = 0;
-    uint32_t aphase = 0, gphase = 0;
+    uint32_t aphase = 0, gphase = 0, oseq = 0;
     Tile tl;
-    for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+    // accumulator released: one arrive per epilogue warp, in a pair on the LEADER's barrier (it gates the next MMAs)
+    auto release_acc = [&](int a) {
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        if (PAIR) mbar_arrive_cluster(mapa_shared(tempty0 + 8 * a, 0));
+        else mbar_arrive(tempty0 + 8 * a);
+      }
+    };
+    Tile nx;
+    bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+    for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
+      okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
       const bool have = tl.nkb > 0;
       const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + as * BN;
       if (MODE == TC_DGRAD_SWIGLU) {
         const int64_t row = (int64_t)tl.m0 + row_in_tile;
         const bool row_ok = row < p.rows_valid;
-        {   // pull the NEXT tile's g, u rows into L2 a whole tile ahead (ch 0 warps take g, ch 1 warps take u)
-          Tile nx;
-          if (decode_tile<MODE>(p, t + gridDim.x, total, nx)) {
-            const int64_t nrow = (int64_t)nx.m0 + row_in_tile;
-            if (nrow < p.rows_valid) {
-              const __nv_bfloat16* src = p.gu + nrow * p.ldgu + (ch ? p.F : 0) + nx.n0;
-              const int ncol = min(BN, p.F - nx.n0);
-              for (int c = 0; c < ncol; c += 64) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + c));
-            }
-          }
-        }
         constexpr int NC = BN / 64;              // chunks per warp: this warp drains columns [ch * 128, ch * 128 + 128)
         if (p.tma_out) {
           const bool issuer = (threadIdx.x & 127) == 64;
-          const uint32_t obuf = obuf0 + ch * OBUF_BYTES, gbar = gbar0 + 8 * ch;
+          const uint32_t obuf = obuf0 + ch * GROUP_OBUF, gbar = gbar0 + 8 * ch;
           const int nvalid = min(NC, (p.F - tl.n0 - ch * (BN / 2) + 31) / 32);      // chunks of this group inside F
           if (issuer && nvalid > 0) gu_tma_fetch(p, tl, ch * NC, obuf, gbar, &tmB1);   // overlaps the rest of the main loop
           __syncwarp();
@@ -635,9 +715,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             if (issuer && i + 1 < nvalid) gu_tma_fetch(p, tl, ch * NC + i + 1, obuf, gbar, &tmB1);
             __syncwarp();
           }
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+          release_acc(as);
           if (++as == 2) { as = 0; aphase ^= 1; }
           continue;
         }
@@ -649,7 +727,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           if (i + 2 < NC) gu_load(p, tl, row, row_ok, ch * NC + i + 2, k[(i + 2) % 3]);
-          dgrad_swiglu_chunk(p, tl, row, row_ok, ch * NC + i, tacc, k[i % 3], obuf0 + ch * OBUF_BYTES, row_in_tile, &tmO,
+          dgrad_swiglu_chunk(p, tl, row, row_ok, ch * NC + i, tacc, k[i % 3], obuf0 + ch * GROUP_OBUF, row_in_tile, &tmO,
                              (threadIdx.x & 127) == 64, ch);
         }
       } else if (MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD) {
@@ -657,16 +735,20 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           mbar_wait(tfull0 + 8 * as, aphase);
           tc_fence_after();
         }
+        // the accumulator is released inside, right after its last TMEM load (one arrive per warp)
+        auto rel = [&]() { if (have) release_acc(as); };
         if (MODE == TC_WGRAD && p.acc_f32) {
-          if (have) wgrad_accum_tile(p, tl, tacc, row_in_tile, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch);
+          if (have) wgrad_accum_tile<NOBUF>(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch, oseq, rel);
         } else {
-          wgrad_store_tile(p, tl, tacc, row_in_tile, have, obuf0 + ch * OBUF_BYTES, &tmO, (threadIdx.x & 127) == 64, ch,
-                           MODE == TC_WGRAD ? tl.e : 0);
+          wgrad_store_tile<NOBUF>(p, tl, tacc, row_in_tile, have, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch,
+                                  MODE == TC_WGRAD ? tl.e : 0, oseq, rel);
         }
+        if (have && ++as == 2) { as = 0; aphase ^= 1; }
+        continue;
       } else if (MODE == TC_FWD_SWIGLU && p.tma_out) {
         mbar_wait(tfull0 + 8 * as, aphase);
         tc_fence_after();
-        fwd_swiglu_tile_tma(p, tl, tacc, row_in_tile, obuf0 + ch * OBUF_BYTES, &tmO, &tmO2, (threadIdx.x & 127) == 64, ch);
+        fwd_swiglu_tile_tma(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, &tmO2, (threadIdx.x & 127) == 64, ch);
       } else {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
@@ -675,9 +757,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         epilogue_tile<MODE>(p, tl, tacc, row_in_tile, have, ch);
       }
       if (have) {
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+        release_acc(as);
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
@@ -686,8 +766,13 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       bulk_wait0();   // all TMA stores complete before the CTA retires
   }
   tc_fence_before();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+  __syncwarp();
+  if (PAIR) cluster_sync_all();   // neither CTA retires (nor frees tensor memory) while its peer may still use it
+  else __syncthreads();
+  if (warp == 1) {
+    if (PAIR) tmem_dealloc_pair(tmem_base, TMEM_COLS);
+    else tmem_dealloc(tmem_base, TMEM_COLS);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -699,38 +784,98 @@ bool make_map(CUtensorMap* m, const void* ptr, int64_t inner, int64_t outer, int
   return tc_make_map(m, 2, ptr, inner, outer, ld, BK, box_outer);
 }
 
-bool g_attr_set[MAX_DEVICES][6];   // per device: cudaFuncAttributeMaxDynamicSharedMemorySize raised for tc_gemm_kernel<MODE>
+bool g_attr_set[MAX_DEVICES][6][2];   // per device: cudaFuncAttributeMaxDynamicSharedMemorySize raised for tc_gemm_kernel<MODE, PAIR>
 
-template <int MODE>
+// max_units = upper bound on tiles (PAIR: pair-tiles).  PAIR launches clusters of two CTAs (one TPC each).
+template <int MODE, bool PAIR>
 int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
-               int64_t max_tiles, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
+               int64_t max_units, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
   const int dev = current_device();
   if (dev < 0) return MOE_ERR_CUDA;
-  if (!g_attr_set[dev][MODE]) {
-    MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    g_attr_set[dev][MODE] = true;
+  if (!g_attr_set[dev][MODE][PAIR]) {
+    MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    g_attr_set[dev][MODE][PAIR] = true;
   }
   const int sms = device_sm_count();
   if (sms <= 0) return MOE_ERR_CUDA;
-  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_tiles));
-  MOE_LAUNCH(tc_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, p);
+  if (!PAIR) {
+    const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_units));
+    MOE_LAUNCH((tc_gemm_kernel<MODE, false>), grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, p);
+    return MOE_OK;
+  }
+  const unsigned pairs = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms / 2, max_units));
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(2 * pairs);
+  cfg.blockDim = dim3(NTHREADS);
+  cfg.dynamicSmemBytes = SMEM_BYTES;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const CUtensorMap& oo2 = o2 ? *o2 : o;
+  ++g_launches;
+  if (cudaLaunchKernelEx(&cfg, tc_gemm_kernel<MODE, true>, a, b0, b1, o, oo2, p) != cudaSuccess) {
+    cudaGetLastError();
+    return MOE_ERR_CUDA;
+  }
   return MOE_OK;
 }
 
-// mtile[0] = number of 128-row tiles below offsets[E]; mtile[1 + i] = expert owning tile i.
-__global__ void prepare_tiles_kernel(const int32_t* __restrict__ offsets, int E, int32_t* __restrict__ mtile) {
-  for (int e = threadIdx.x; e < E; e += blockDim.x) {
-    const int lo = offsets[e] / BM, hi = offsets[e + 1] / BM;
-    for (int t = lo; t < hi; ++t) mtile[1 + t] = e;
+// Which launches use the CTA-pair kernel.  Default 1: the weight gradients (no ragged dimension: every 256 x 256 tile
+// is a full pair tile) and single-group GEMMs (shared expert, router); the ragged expert GEMMs stay on the 1-CTA kernel
+// because the unpaired last M-tile of every other expert needs a second launch whose tail costs what the pairs save
+// (measured).  Debug knob, not part of the ABI: MOE_B200_PAIR=0 (never) / 1 / 2 (ragged GEMMs too).
+int pair_mode() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = getenv("MOE_B200_PAIR");
+    v = (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
   }
-  if (threadIdx.x == 0) mtile[0] = offsets[E] / BM;
+  return v;
+}
+
+// One logical GEMM = the pair kernel over the paired M-tiles (or over everything: single group, wgrad) followed by the
+// 1-CTA kernel over the unpaired M-tiles.  With `pl == nullptr` (no pair table) the 1-CTA kernel runs all tiles.
+template <int MODE>
+int32_t launch_both(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b0_pair, const CUtensorMap& b1,
+                    const CUtensorMap& o, TcParams p, const TcCall& c, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
+  const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
+  const bool grouped = c.mtile != nullptr;
+  if (pair_mode() == 0 || (grouped && (pair_mode() < 2 || !c.plist || !c.olist))) {
+    p.tlist = nullptr;
+    return launch<MODE, false>(a, b0, b1, o, p, max_mtiles * p.n_tiles, s, o2);
+  }
+  if (!grouped) {       // one group of rows_cap rows from row 0: pairs of consecutive M-tiles cover it
+    p.tlist = nullptr;
+    return launch<MODE, true>(a, b0_pair, b1, o, p, ceil_div(c.rows_cap, 2 * BM) * p.n_tiles, s, o2);
+  }
+  p.tlist = c.plist;
+  MOE_CHECK((launch<MODE, true>(a, b0_pair, b1, o, p, (max_mtiles / 2) * p.n_tiles, s, o2)));
+  p.tlist = c.olist;
+  return launch<MODE, false>(a, b0, b1, o, p, (int64_t)std::min<int64_t>(c.E, max_mtiles) * p.n_tiles, s, o2);
+}
+
+// Tile tables (tile_tables.cuh) from the row offsets alone, for the stand-alone grouped-GEMM entry points.
+__global__ void __launch_bounds__(1024) prepare_tiles_kernel(const int32_t* __restrict__ offsets, int E,
+                                                             int32_t* __restrict__ mtile, int32_t* __restrict__ plist,
+                                                             int32_t* __restrict__ olist) {
+  __shared__ int32_t wsum[32];
+  const int e = threadIdx.x;
+  const int excl = e < E ? offsets[e] : 0, incl = e < E ? offsets[e + 1] : 0;
+  write_tile_tables(e, E, excl, incl, mtile, plist, olist, wsum);
 }
 
 }  // namespace
 
 int32_t tc_prepare_tiles(const int32_t* offsets, int E, int64_t rows_cap, int32_t* mtile_expert, cudaStream_t s) {
-  (void)rows_cap;
-  MOE_LAUNCH(prepare_tiles_kernel, 1, 256, 0, s, offsets, E, mtile_expert);
+  if (E > 1024) return MOE_ERR_UNSUPPORTED;
+  MOE_LAUNCH(prepare_tiles_kernel, 1, 1024, 0, s, offsets, E, mtile_expert, mtile_expert + tile_plist_off(rows_cap),
+             mtile_expert + tile_olist_off(rows_cap));
   return MOE_OK;
 }
 
@@ -742,6 +887,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.rows_valid = c.rows_cap;
   p.mtile = c.mtile;
   p.offsets = c.offsets;
+  p.counts = c.counts;
   p.out0 = (__nv_bfloat16*)c.out0;
   p.ld0 = c.ld0;
   p.out1 = (__nv_bfloat16*)c.out1;
@@ -753,8 +899,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.M = c.M;
   p.b_rows = c.b_rows;
   p.a_col0 = c.a_col0;
-  CUtensorMap ta, tb0, tb1, to;
-  const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
+  CUtensorMap ta, tb0, tb0p, tb1, to;
   if (c.mode == TC_FWD_F32 ? ((c.N & 3) || (c.ld0 & 3)) : ((c.N & 7) || (c.ld0 & 7))) return MOE_ERR_UNSUPPORTED;
   switch (c.mode) {
     case TC_FWD_F32:
@@ -764,9 +909,10 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       p.n_tiles = (int)ceil_div(c.N, BN);
       if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
-      if (c.mode == TC_FWD_F32) return launch<TC_FWD_F32>(ta, tb0, tb0, ta, p, max_mtiles * p.n_tiles, s);
+      if (!make_map(&tb0p, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;   // a pair CTA's half
+      if (c.mode == TC_FWD_F32) return launch_both<TC_FWD_F32>(ta, tb0, tb0p, tb0, ta, p, c, s);
       if (!tc_make_map3(&to, 2, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // C [rows, N]
-      return launch<TC_FWD>(ta, tb0, tb0, to, p, max_mtiles * p.n_tiles, s);
+      return launch_both<TC_FWD>(ta, tb0, tb0p, tb0, to, p, c, s);
     }
     case TC_FWD_SWIGLU: {
       if (c.Kd % BK || (c.F & 7) || (c.ld1 & 7)) return MOE_ERR_UNSUPPORTED;
@@ -780,8 +926,8 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (p.tma_out && (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM) ||    // gu [rows, 2F]
                         !tc_make_map3(&to2, 2, c.out1, c.F, c.rows_cap, 1, c.ld1, 32, BM)))                  // a [rows, F]
         p.tma_out = 0;
-      if (!p.tma_out) return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, ta, p, max_mtiles * p.n_tiles, s);
-      return launch<TC_FWD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s, &to2);
+      if (!p.tma_out) return launch_both<TC_FWD_SWIGLU>(ta, tb0, tb0, tb1, ta, p, c, s);
+      return launch_both<TC_FWD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s, &to2);
     }
     case TC_DGRAD:
     case TC_DGRAD_SWIGLU: {
@@ -796,7 +942,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (!make_map(&tb1, split ? c.B1 : c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (c.mode == TC_DGRAD) {
         if (!tc_make_map3(&to, 2, c.out0, c.N, c.rows_cap, 1, c.ld0, 64, BM)) return MOE_ERR_UNSUPPORTED;   // dA [rows, N]
-        return launch<TC_DGRAD>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
+        return launch_both<TC_DGRAD>(ta, tb0, tb0, tb1, to, p, c, s);
       }
       if ((c.F & 7) || (c.ldgu & 7)) return MOE_ERR_UNSUPPORTED;
       p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // dg / du boxes of 32 columns must not straddle the [dg|du] boundary
@@ -804,19 +950,28 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
           !tc_make_map3(&tb1, 2, c.gu, 2 * (int64_t)c.F, c.rows_cap, 1, c.ldgu, 32, BM))
         p.tma_out = 0;
       if (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
-      return launch<TC_DGRAD_SWIGLU>(ta, tb0, tb1, to, p, max_mtiles * p.n_tiles, s);
+      return launch_both<TC_DGRAD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s);
     }
     case TC_WGRAD: {
-      p.m_tiles = (int)ceil_div(c.M, BM);
+      // every (expert, 256 x 256 output tile) goes to a CTA pair: no ragged dimension, the contraction runs over the
+      // expert's rows.  A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (output columns).
+      // The pair kernel pays where operand traffic binds: contractions of >= 4 k-blocks (about 256 real rows per expert;
+      // rows_cap counts 127 padding rows per expert) and an output height that 256-row tiles cover without extra padding.
+      // Measured: configs[1] 690 -> 625 us; configs[2] (128 rows per expert: 2 k-blocks per 64 KB of
+      // output per CTA, write-bound) 8.04 -> 8.75 ms and configs[4] (2880 = 11.25 x 256) 4.2 -> 4.5 ms, so those stay 1-CTA.
+      const bool pair = pair_mode() > 0 && (c.mtile == nullptr || c.rows_cap >= 384 * (int64_t)c.E) &&
+                        ceil_div(c.M, 2 * BM) * 2 == ceil_div(c.M, BM);
+      p.m_tiles = (int)ceil_div(c.M, pair ? 2 * BM : BM);
       p.n_tiles = (int)ceil_div(c.N, BN);
-      // A: [rows_cap, lda] read MN-major (inner = columns = output rows); A2 likewise (inner = output columns)
       if (!make_map(&ta, c.A, c.lda, c.rows_cap, c.lda, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.A2, c.N, c.rows_cap, c.lda2, 64)) return MOE_ERR_UNSUPPORTED;
       p.acc_f32 = c.acc_f32 ? 1 : 0;
       if (c.acc_f32 ? !tc_make_map3(&to, 4, c.out0, c.N, c.M, c.E, c.ld0, 32, BM)    // fp32 dB [E, M, N], reduce-add
                     : !tc_make_map3(&to, 2, c.out0, c.N, c.M, c.E, c.ld0, 64, BM))   // bf16 dB [E, M, N], overwrite
         return MOE_ERR_UNSUPPORTED;
-      return launch<TC_WGRAD>(ta, tb0, tb0, to, p, (int64_t)c.E * p.m_tiles * p.n_tiles, s);
+      const int64_t units = (int64_t)c.E * p.m_tiles * p.n_tiles;
+      if (pair) return launch<TC_WGRAD, true>(ta, tb0, tb0, to, p, units, s);
+      return launch<TC_WGRAD, false>(ta, tb0, tb0, to, p, units, s);
     }
   }
   return MOE_ERR_INVALID_ARG;

@@ -19,8 +19,11 @@ struct TcCall {
   int mode;
   int E;                   // groups
   int64_t rows_cap;        // height of the row-grouped buffers (TMA bound; rows >= it read as zero)
+  const int32_t* counts;   // [E] device or nullptr: real rows per group (WGRAD trims its contraction to them)
   const int32_t* offsets;  // [E+1] device; group e = rows [offsets[e], offsets[e+1]), multiples of 128 if mtile != nullptr
   const int32_t* mtile;    // device {n_tiles, expert of tile 0, ...} or nullptr: one group of rows_cap rows at row 0
+  const int32_t* plist;    // device pair / unpaired M-tile lists (tile_tables.cuh) belonging to mtile, or nullptr:
+  const int32_t* olist;    //   then every tile runs on the 1-CTA kernel
   // --- operands (device, bf16) ---
   const void* A;  int lda;   // row-grouped left operand            [rows_cap, lda]
   const void* B0; const void* B1;  // weights [E, b_rows, b_cols] (B1: Wu for FWD_SWIGLU / second half of split DGRAD)

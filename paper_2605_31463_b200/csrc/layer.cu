@@ -5,6 +5,7 @@
 
 #include "fp8.cuh"
 #include "gemm_tc.cuh"
+#include "tile_tables.cuh"
 
 namespace moe {
 
@@ -39,7 +40,12 @@ TcCall tc_base(const FfnGroup& g, int mode) {
   c.E = g.E;
   c.rows_cap = g.rows_cap;
   c.offsets = g.offsets;
+  c.counts = g.mtile ? g.counts : nullptr;
   c.mtile = g.mtile;
+  if (g.mtile) {            // the pair / unpaired lists sit behind the M-tile table (tile_tables.cuh)
+    c.plist = g.mtile + tile_plist_off(g.rows_cap);
+    c.olist = g.mtile + tile_olist_off(g.rows_cap);
+  }
   c.F = g.F;
   return c;
 }

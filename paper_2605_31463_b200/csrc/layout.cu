@@ -2,6 +2,7 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "tile_tables.cuh"
 
 namespace moe {
 
@@ -69,7 +70,7 @@ CtxLayout ctx_layout(const moe_config_t* c) {
   L.offsets = k.take((E + 1) * 4 + 16);  // + {0, T} for the shared expert's single group
   L.p2f = k.take(R * 4);
   L.f2p = k.take(T * c->K * 4);
-  L.mtile = k.take((R / 128 + 4) * 4);
+  L.mtile = k.take(tile_table_ints((int64_t)R, c->E) * 4);   // mtile | plist | olist (tile_tables.cuh)
   L.Xp = k.take(R * H * es);
   L.gu = k.take(R * 2 * F * es);
   L.a = k.take(R * F * es);
@@ -106,7 +107,7 @@ WsLayout ws_layout(const moe_config_t* c) {
   const size_t nchunks = (T * c->K + PERM_CHUNK - 1) / PERM_CHUNK;
   L.hist = k.take(nchunks * E * 4);
   // tmp: M-tile table for stand-alone calls, or da [R,F] / da_s [T,Fs] on the CUDA-core path
-  size_t tmp = (R / 128 + 4) * 4;
+  size_t tmp = tile_table_ints((int64_t)R, c->E) * 4;
   if (R * F * es > tmp) tmp = R * F * es;
   if (T * Fs * es > tmp) tmp = T * Fs * es;
   L.tmp = k.take(tmp);

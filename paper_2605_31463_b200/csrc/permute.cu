@@ -3,6 +3,7 @@
 // No atomics anywhere: ranks come from warp match/ballot and per-chunk prefix tables, so the maps are
 // deterministic and bit-exact against the oracle's stable counting sort.
 #include "common.cuh"
+#include "tile_tables.cuh"
 
 namespace moe {
 namespace {
@@ -51,11 +52,11 @@ __global__ void __launch_bounds__(CHUNK_WARPS * 32) hist_kernel(const int32_t* _
 }
 
 // Phase 2 (one CTA of 1024 threads): counts, aligned exclusive offsets, per-chunk bases (in place in
-// hist), and the M-tile -> expert table used by the tensor-core GEMMs (mtile[0] = number of 128-row
-// tiles, mtile[1 + i] = expert of tile i) when row_align is a multiple of 128.
+// hist), and the tile tables of the tensor-core GEMMs (tile_tables.cuh) when row_align is a multiple of 128.
 __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, int nchunks, int E, int row_align,
                                                     int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
-                                                    int32_t* __restrict__ mtile) {
+                                                    int32_t* __restrict__ mtile, int32_t* __restrict__ plist,
+                                                    int32_t* __restrict__ olist) {
   __shared__ int32_t wsum[32];
   const int e = threadIdx.x;
   int cnt = 0;
@@ -63,27 +64,7 @@ __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, 
     for (int c = 0; c < nchunks; ++c) cnt += hist[(size_t)c * E + e];
   const int a = row_align < 1 ? 1 : row_align;
   const int padded = (e < E) ? (cnt + a - 1) / a * a : 0;
-  // block-wide exclusive scan of `padded`
-  const int lane = e & 31, warp = e >> 5;
-  int v = padded;
-#pragma unroll
-  for (int off = 1; off < 32; off <<= 1) {
-    const int o = __shfl_up_sync(FULL, v, off);
-    if (lane >= off) v += o;
-  }
-  if (lane == 31) wsum[warp] = v;
-  __syncthreads();
-  if (warp == 0) {
-    int ws = wsum[lane];
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-      const int o = __shfl_up_sync(FULL, ws, off);
-      if (lane >= off) ws += o;
-    }
-    wsum[lane] = ws;
-  }
-  __syncthreads();
-  const int incl = v + (warp > 0 ? wsum[warp - 1] : 0);
+  const int incl = block_incl_scan_1024(padded, wsum);
   const int excl = incl - padded;
   if (e < E) {
     counts[e] = cnt;
@@ -95,11 +76,8 @@ __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, 
       hist[(size_t)c * E + e] = run;
       run += h;
     }
-    if (mtile != nullptr) {
-      for (int t = excl / 128; t < incl / 128; ++t) mtile[1 + t] = e;
-      if (e == E - 1) mtile[0] = incl / 128;
-    }
   }
+  if (mtile != nullptr) write_tile_tables(e, E, excl, incl, mtile, plist, olist, wsum);
 }
 
 // Phase 3: scatter.  flat_to_perm[p] = base[chunk][e] + rank of p among the chunk's positions of e.
@@ -148,7 +126,9 @@ int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, i
   MOE_CUDA(cudaMemsetAsync(p2f, 0xFF, (size_t)padded_rows(c) * sizeof(int32_t), s));
   MOE_LAUNCH(hist_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist);
   int32_t* mt = (c->row_align % 128 == 0) ? mtile_expert : nullptr;
-  MOE_LAUNCH(scan_kernel, 1, 1024, 0, s, hist, nchunks, c->E, c->row_align, counts, offsets, mt);
+  const int64_t R = padded_rows(c);
+  MOE_LAUNCH(scan_kernel, 1, 1024, 0, s, hist, nchunks, c->E, c->row_align, counts, offsets, mt,
+             mt ? mt + tile_plist_off(R) : nullptr, mt ? mt + tile_olist_off(R) : nullptr);
   MOE_LAUNCH(scatter_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist, p2f, f2p);
   return MOE_OK;
 }
