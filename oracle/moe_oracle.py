@@ -15,6 +15,11 @@ NumPy fp64, in the order and notation of SURVEY.md §8(c) R1..R9.  The paper its
 Every other choice is a reading listed in DESIGN.md ("Readings of the paper"), taken from
 SURVEY.md §8(c) S1..S20 and BASELINE.json:north_star / configs.
 
+Widened rows (readings A1..A3, V1, V2 of DESIGN.md section 2): the auxiliary global-level
+load-balancing loss, the threshold-gated variable-k router and the
+zero-computation experts.  They are off unless the config enables them
+(aux_coef != 0, route_mode == 1, n_zero + n_copy + n_const > 0).
+
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): brute-force top-k with hand-made ties; weight
 sum / sign; softmax->top-k->renorm == top-k->softmax closed form; group-limit
 reductions; permutation bijection / stability; permute->combine identity with w = 1/K; E=1,K=1 ==
@@ -122,15 +127,107 @@ def gate_weights(z, idx, cfg):
     return c * s
 
 
-def route(z, bias, cfg, key_dtype=F64, forced_idx=None):
+def threshold_select(key, thr, K):
+    """V1: an expert is active for a token iff its gate s = sigmoid(z) exceeds the expert's
+    threshold thr[e]; the number of active experts varies per token.  Active experts fill the K slots in
+    (s desc, index asc) order (more than K active: the K largest stay); unused slots hold -1; a token no expert
+    admits keeps its single best expert (top-1 fallback), so every token is computed (dropless)."""
+    key = np.asarray(key)
+    T, E = key.shape
+    act = key > np.asarray(thr).astype(key.dtype)[None, :]
+    masked = np.where(act, key, np.asarray(NEG_INF, key.dtype))
+    idx = topk_select(masked, K)                               # inactive experts have key -inf
+    n_act = act.sum(axis=1)
+    idx = np.where(np.arange(K)[None, :] < n_act[:, None], idx, -1).astype(np.int32)   # slot j is filled iff j < #active
+    none = n_act == 0
+    idx[none, 0] = np.argmax(key[none], axis=1)               # first maximal index: ties -> lower expert
+    return idx
+
+
+def gate_weights_masked(z, idx, cfg):
+    """R5 over a variable-size selection (slots with idx = -1 are empty: weight 0).  Sigmoid scores only (V1)."""
+    z = np.asarray(z, F64)
+    ok = idx >= 0
+    s = np.where(ok, sigmoid(np.take_along_axis(z, np.where(ok, idx, 0).astype(np.int64), axis=1)), 0.0)
+    c = float(cfg.routed_scale)
+    if cfg.renorm:
+        return c * s / (s.sum(axis=1, keepdims=True) + 1e-20)
+    return c * s
+
+
+def route(z, bias, cfg, key_dtype=F64, forced_idx=None, threshold=None):
     """R2..R5: (topk_idx int32 [T,K], topk_w fp64 [T,K]).  `forced_idx` overrides the selection
-    (used by parity tests only for tokens whose k/(k+1) key gap is a verified near-tie)."""
+    (used by parity tests only for tokens whose k/(k+1) key gap is a verified near-tie).
+    route_mode 1 (V1): threshold-gated variable-k selection on the sigmoid gates; `threshold` is thr[E]."""
+    if getattr(cfg, "route_mode", 0) == 1:
+        if forced_idx is None:
+            idx = threshold_select(sigmoid(z).astype(key_dtype), threshold, cfg.K)
+        else:
+            idx = np.asarray(forced_idx, np.int32)
+        return idx, gate_weights_masked(z, idx, cfg)
     if forced_idx is None:
         key = group_limit(selection_keys(z, bias, cfg, key_dtype), cfg)
         idx = topk_select(key, cfg.K)
     else:
         idx = np.asarray(forced_idx, np.int32)
     return idx, gate_weights(z, idx, cfg)
+
+
+# =====================================================================================
+# A1..A3  auxiliary global-level load-balancing loss          (PAPER.md:349-350; [30])
+# =====================================================================================
+
+
+def router_probs(z, cfg):
+    """A2: the differentiable per-token distribution over ALL experts that the balance term averages:
+    softmax configs p = softmax(z); sigmoid configs p = s / sum_e s (normalised gate scores)."""
+    z = np.asarray(z, F64)
+    if cfg.score_fn == 0 and getattr(cfg, "route_mode", 0) == 0:
+        m = z.max(axis=1, keepdims=True)
+        p = np.exp(z - m)
+    else:
+        p = sigmoid(z)
+    return p / p.sum(axis=1, keepdims=True)
+
+
+def aux_expert_weights(cfg):
+    """V2 (PAPER.md:488 R3): zero-computation experts enter the balance term with weight aux_zc_weight, FFN experts 1."""
+    eta = np.ones(cfg.E, F64)
+    nz = cfg.n_zero + cfg.n_copy + cfg.n_const
+    if nz:
+        eta[cfg.E - nz:] = float(cfg.aux_zc_weight)
+    return eta
+
+
+def aux_loss(cfg, z, idx, f_global=None):
+    """A1: L_aux = aux_coef * E * sum_e eta_e f_e P_e with f_e = the fraction of the batch's routed assignments that
+    went to expert e (counted over the GLOBAL batch: `f_global` when the caller has all-reduced the counts over its
+    data-parallel ranks, else this batch's own counts; variable-k routing divides by the number of assignments made,
+    PAPER.md:456) and P_e = mean over tokens of p[t, e].  f carries no gradient.  Returns (loss, f, P)."""
+    E = cfg.E
+    if f_global is None:
+        flat = np.asarray(idx).reshape(-1)
+        flat = flat[flat >= 0]
+        f = np.bincount(flat, minlength=E).astype(F64) / max(flat.size, 1)
+    else:
+        f = np.asarray(f_global, F64)
+    P = router_probs(z, cfg).mean(axis=0)
+    return float(cfg.aux_coef) * E * float((aux_expert_weights(cfg) * f * P).sum()), f, P
+
+
+def aux_dz(cfg, z, f):
+    """A3: d L_aux / d z[t, j] (dense [T,E]).  softmax: (c/T) p_j (g_j - sum_e g_e p_e); normalised sigmoid:
+    (c/T) s_j (1 - s_j) / S (g_j - sum_e g_e p_e); c = aux_coef * E, g = eta * f."""
+    z = np.asarray(z, F64)
+    T = z.shape[0]
+    p = router_probs(z, cfg)
+    g = aux_expert_weights(cfg) * np.asarray(f, F64)
+    inner = (p * g[None, :]).sum(axis=1, keepdims=True)
+    c = float(cfg.aux_coef) * cfg.E / T
+    if cfg.score_fn == 0 and getattr(cfg, "route_mode", 0) == 0:
+        return c * p * (g[None, :] - inner)
+    s = sigmoid(z)
+    return c * s * (1.0 - s) / s.sum(axis=1, keepdims=True) * (g[None, :] - inner)
 
 
 # =====================================================================================
@@ -143,15 +240,15 @@ def permute_maps(idx, E, row_align=1):
     Flat position p = t*K + j.  Within an expert rows are in ascending p.  Each group starts at a
     multiple of row_align; padding rows map to -1."""
     flat = np.asarray(idx, np.int64).reshape(-1)
-    counts = np.bincount(flat, minlength=E).astype(np.int32)
+    counts = np.bincount(flat[flat >= 0], minlength=E).astype(np.int32)   # -1 = empty slot (variable-k routing, V1)
     a = max(int(row_align), 1)
     padded = (counts.astype(np.int64) + a - 1) // a * a
     offsets = np.zeros(E + 1, np.int64)
     offsets[1:] = np.cumsum(padded)
     perm_to_flat = np.full(int(offsets[E]), -1, np.int32)
-    flat_to_perm = np.empty(flat.size, np.int32)
+    flat_to_perm = np.full(flat.size, -1, np.int32)
     order = np.argsort(flat, kind="stable")          # ascending expert, then ascending p
-    start = 0
+    start = int((flat < 0).sum())                    # empty slots sort first and are skipped
     for e in range(E):
         c = int(counts[e])
         p = order[start:start + c]
@@ -178,7 +275,8 @@ def unpermute_combine(y, w, flat_to_perm, shared_out=None):
     Y = np.zeros((T, y.shape[1]), F64)
     f2p = flat_to_perm.reshape(T, K)
     for j in range(K):
-        Y += np.asarray(w, F64)[:, j:j + 1] * y[f2p[:, j]]
+        ok = f2p[:, j] >= 0                          # empty slot: no row, no contribution
+        Y[ok] += np.asarray(w, F64)[ok, j:j + 1] * y[f2p[ok, j]]
     if shared_out is not None:
         Y += np.asarray(shared_out, F64)
     return Y
@@ -385,13 +483,29 @@ def _expert_weights(W, e):
     return W[0][e], W[1][e], W[2][e]
 
 
-def layer_fwd(cfg, X, Wr, bias, W, shared=None, forced_idx=None, key_dtype=F64):
+def zc_kind(cfg, e):
+    """V2: the last n_zero + n_copy + n_const router outputs are zero-computation experts, in that order.
+    Returns None for an FFN expert, else ("zero" | "copy" | "const", index within its kind)."""
+    nz = cfg.n_zero + cfg.n_copy + cfg.n_const
+    j = e - (cfg.E - nz)
+    if j < 0:
+        return None
+    if j < cfg.n_zero:
+        return "zero", j
+    if j < cfg.n_zero + cfg.n_copy:
+        return "copy", j - cfg.n_zero
+    return "const", j - cfg.n_zero - cfg.n_copy
+
+
+def layer_fwd(cfg, X, Wr, bias, W, shared=None, forced_idx=None, key_dtype=F64, extras=None):
     """Forward of the routed-expert layer.  Returns a dict with every intermediate in fp64
-    (permuted-row tensors use the R6 layout for cfg.row_align)."""
+    (permuted-row tensors use the R6 layout for cfg.row_align).  `extras` (widened rows): threshold [E] (V1),
+    zc_const [n_const, H] (V2), f_global [E] (A1).  W holds the E - n_zc FFN experts."""
+    extras = extras or {}
     fp8 = cfg.dtype == 2
     mode = cfg.fp8_scale_mode
     z = router_logits(X, Wr)
-    idx, w = route(z, bias, cfg, key_dtype, forced_idx)
+    idx, w = route(z, bias, cfg, key_dtype, forced_idx, threshold=extras.get("threshold"))
     counts, offsets, p2f, f2p = permute_maps(idx, cfg.E, cfg.row_align)
     Xin = fq_act(X, mode) if fp8 else np.asarray(X, F64)      # Q-X: once per token, then permuted
     Xp = permute_rows(Xin, p2f, cfg.K)
@@ -401,6 +515,13 @@ def layer_fwd(cfg, X, Wr, bias, W, shared=None, forced_idx=None, key_dtype=F64):
     for e in range(cfg.E):
         lo, c = int(offsets[e]), int(counts[e])
         if c == 0:
+            continue
+        kind = zc_kind(cfg, e)
+        if kind is not None:                                   # V2: no FFN; y = 0 | the token's own (bf16) row | the constant vector
+            if kind[0] == "copy":
+                y[lo:lo + c] = permute_rows(np.asarray(X, F64), p2f, cfg.K)[lo:lo + c]
+            elif kind[0] == "const":
+                y[lo:lo + c] = np.asarray(extras["zc_const"], F64)[kind[1]][None, :]
             continue
         Wg, Wu, Wd = _expert_weights(W, e)
         if fp8:
@@ -416,48 +537,58 @@ def layer_fwd(cfg, X, Wr, bias, W, shared=None, forced_idx=None, key_dtype=F64):
             sg, su, sa, sy = expert_ffn_fwd(X, *shared)
         sh = dict(g=sg, u=su, a=sa, y=sy)
     Y = unpermute_combine(y, w, f2p, None if sh is None else sh["y"])
-    return dict(z=z, idx=idx, w=w, counts=counts, offsets=offsets, perm_to_flat=p2f, flat_to_perm=f2p,
-                Xp=Xp, g=g, u=u, a=a, y=y, shared=sh, Y=Y)
+    out = dict(z=z, idx=idx, w=w, counts=counts, offsets=offsets, perm_to_flat=p2f, flat_to_perm=f2p,
+               Xp=Xp, g=g, u=u, a=a, y=y, shared=sh, Y=Y)
+    if getattr(cfg, "aux_coef", 0.0):
+        out["aux_loss"], out["aux_f"], out["aux_P"] = aux_loss(cfg, z, idx, extras.get("f_global"))
+    return out
 
 
-def router_bwd(cfg, z, idx, w, dw):
-    """R8 router part: dz[T,E] (dense, zero outside the selection) from dw[T,K].
+def router_bwd(cfg, z, idx, w, dw, aux_f=None):
+    """R8 router part: dz[T,E] (dense, zero outside the selection unless stated) from dw[T,K].
     softmax+renorm: dz_j = w_j (dw_j - sum_i w_i dw_i) over the selected set (w here includes the
     constant routed_scale c, which the closed form carries through unchanged).
-    softmax, no renorm: w_j = c*softmax_all(z)_j  =>  dz_e = p_e (c*[e in sel] dw_e - sum_i w_i dw_i).
+    softmax, no renorm: w_j = c*softmax_all(z)_j  =>  dz_e = p_e (c*[e in sel] dw_e - sum_i w_i dw_i)   (dense).
     sigmoid+renorm (S = sum s_i + 1e-20): ds_j = c (dw_j/S - sum_i dw_i s_i / S^2), dz_j = ds_j s_j (1-s_j).
-    sigmoid, no renorm: dz_j = c dw_j s_j (1-s_j).  top-k, group mask and bias carry no gradient."""
+    sigmoid, no renorm: dz_j = c dw_j s_j (1-s_j).  top-k, group mask, bias and thresholds carry no gradient.
+    Empty slots (idx = -1, V1) contribute nothing.  aux_f != None adds the dense gradient of the balance loss (A3)."""
     T, E = z.shape
-    idx64 = idx.astype(np.int64)
+    ok = np.asarray(idx) >= 0
+    idx64 = np.where(ok, idx, 0).astype(np.int64)
     dz = np.zeros((T, E), F64)
     c = float(cfg.routed_scale)
-    dw = np.asarray(dw, F64)
-    if cfg.score_fn == 0:
+    dw = np.where(ok, np.asarray(dw, F64), 0.0)
+    w = np.where(ok, np.asarray(w, F64), 0.0)
+    rows = np.nonzero(ok)
+
+    def put(vals):
+        dz[rows[0], idx64[ok]] += vals[ok]
+
+    if cfg.score_fn == 0 and getattr(cfg, "route_mode", 0) == 0:
         if cfg.renorm:
-            dzs = w * (dw - (w * dw).sum(axis=1, keepdims=True) / c) if c != 0 else np.zeros_like(w)
-            np.put_along_axis(dz, idx64, dzs, axis=1)
+            put(w * (dw - (w * dw).sum(axis=1, keepdims=True) / c) if c != 0 else np.zeros_like(w))
         else:
             m = z.max(axis=1, keepdims=True)
             p = np.exp(z - m); p /= p.sum(axis=1, keepdims=True)
-            inner = (w * dw).sum(axis=1, keepdims=True)          # sum_i c p_i dw_i over selected
-            dz = -p * inner
-            dzs = np.take_along_axis(dz, idx64, axis=1) + w * dw
-            np.put_along_axis(dz, idx64, dzs, axis=1)
-        return dz
-    zs = np.take_along_axis(np.asarray(z, F64), idx64, axis=1)
-    s = sigmoid(zs)
-    if cfg.renorm:
-        S = s.sum(axis=1, keepdims=True) + 1e-20
-        ds = c * (dw / S - (dw * s).sum(axis=1, keepdims=True) / S ** 2)
+            dz = -p * (w * dw).sum(axis=1, keepdims=True)        # sum_i c p_i dw_i over selected
+            put(w * dw)
     else:
-        ds = c * dw
-    np.put_along_axis(dz, idx64, ds * s * (1.0 - s), axis=1)
+        s = np.where(ok, sigmoid(np.take_along_axis(np.asarray(z, F64), idx64, axis=1)), 0.0)
+        if cfg.renorm:
+            S = s.sum(axis=1, keepdims=True) + 1e-20
+            ds = c * (dw / S - (dw * s).sum(axis=1, keepdims=True) / S ** 2)
+        else:
+            ds = c * dw
+        put(ds * s * (1.0 - s))
+    if aux_f is not None and getattr(cfg, "aux_coef", 0.0):
+        dz = dz + aux_dz(cfg, z, aux_f)
     return dz
 
 
-def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None):
-    """Backward for L = sum(Y * dY).  Returns dX, dWr, per-expert dWg/dWu/dWd (stacked), shared grads,
-    and the intermediates dw, dz, dy, dg, du, dXp."""
+def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None, extras=None):
+    """Backward for L = sum(Y * dY) (+ L_aux when aux_coef != 0).  Returns dX, dWr, per-expert dWg/dWu/dWd
+    (stacked over the FFN experts), shared grads, dzc_const (V2) and the intermediates dw, dz, dy, dg, du, dXp."""
+    extras = extras or {}
     fp8 = cfg.dtype == 2
     mode = cfg.fp8_scale_mode
     dY = np.asarray(dY, F64); X64 = np.asarray(X, F64)
@@ -473,19 +604,30 @@ def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None):
     dy = np.zeros((R, cfg.H), F64)
     dy[ok] = wr[ok, None] * dY[tok[ok]]
     f2p2 = f2p.reshape(T, K)
-    dw = np.stack([(dY * fwd["y"][f2p2[:, j]]).sum(axis=1) for j in range(K)], axis=1)   # <dY[t], y_r>
+    dw = np.stack([np.where(f2p2[:, j] >= 0, (dY * fwd["y"][np.maximum(f2p2[:, j], 0)]).sum(axis=1), 0.0)
+                   for j in range(K)], axis=1)                                           # <dY[t], y_r>; empty slot: 0
     dYq = fq_act(dY, mode) if fp8 else None                                    # Q-dY (w applied after the GEMM)
     Xb = np.asarray(X, F64)                                                    # wgrad uses the bf16 tensors
     Xpb = permute_rows(Xb, p2f, K)
     dXp = np.zeros((R, cfg.H), F64)
     dgs = np.zeros((R, cfg.F), F64); dus = np.zeros((R, cfg.F), F64)
-    dWg = np.zeros((E, cfg.F, cfg.H), F64); dWu = np.zeros((E, cfg.F, cfg.H), F64)
-    dWd = np.zeros((E, cfg.H, cfg.F), F64)
+    nzc = cfg.n_zero + cfg.n_copy + cfg.n_const
+    Ef = E - nzc                                                               # FFN experts (V2: the rest compute nothing)
+    dWg = np.zeros((Ef, cfg.F, cfg.H), F64); dWu = np.zeros((Ef, cfg.F, cfg.H), F64)
+    dWd = np.zeros((Ef, cfg.H, cfg.F), F64)
+    dzc = np.zeros((cfg.n_const, cfg.H), F64)
     for e in range(E):
         lo, c = int(offsets[e]), int(counts[e])
         if c == 0:
             continue                                                           # empty expert: dW == 0 exactly
         sl = slice(lo, lo + c)
+        kind = zc_kind(cfg, e)
+        if kind is not None:                                                   # y = 0 | x | v  =>  dXp = 0 | dy | 0, dv = sum dy
+            if kind[0] == "copy":
+                dXp[sl] = dy[sl]
+            elif kind[0] == "const":
+                dzc[kind[1]] = dy[sl].sum(axis=0)
+            continue
         Wg, Wu, Wd = _expert_weights(W, e)
         if fp8:
             dXp[sl], dWg[e], dWu[e], dWd[e], dg, du = expert_ffn_bwd_fp8(
@@ -494,12 +636,13 @@ def layer_bwd(cfg, dY, X, Wr, W, fwd, shared=None):
             dXp[sl], dWg[e], dWu[e], dWd[e], dg, du = expert_ffn_bwd(
                 dy[sl], Xpb[sl], fwd["g"][sl], fwd["u"][sl], fwd["a"][sl], Wg, Wu, Wd)
         dgs[sl], dus[sl] = dg, du
-    dz = router_bwd(cfg, fwd["z"], idx, w, dw)
+    dz = router_bwd(cfg, fwd["z"], idx, w, dw, aux_f=fwd.get("aux_f"))
     dWr = dz.T @ X64
     dX = dz @ np.asarray(Wr, F64)
-    for j in range(K):                                                         # fixed j order
-        dX = dX + dXp[f2p2[:, j]]
-    out = dict(dX=dX, dWr=dWr, dWg=dWg, dWu=dWu, dWd=dWd, dw=dw, dz=dz, dy=dy, dg=dgs, du=dus, dXp=dXp)
+    for j in range(K):                                                         # fixed j order; empty slots skipped
+        okj = f2p2[:, j] >= 0
+        dX[okj] = dX[okj] + dXp[f2p2[okj, j]]
+    out = dict(dX=dX, dWr=dWr, dWg=dWg, dWu=dWu, dWd=dWd, dw=dw, dz=dz, dy=dy, dg=dgs, du=dus, dXp=dXp, dzc_const=dzc)
     if shared is not None:
         sh = fwd["shared"]
         if fp8:

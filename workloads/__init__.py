@@ -45,6 +45,13 @@ class MoEConfig:
     dtype: int = DTYPE_BF16
     fp8_scale_mode: int = 0
     row_align: int = 1
+    # widened rows; all off by default
+    route_mode: int = 0            # 0 = top-k (R2..R5), 1 = threshold-gated variable-k on sigmoid gates
+    n_zero: int = 0                # zero-computation experts: the LAST n_zero + n_copy + n_const of the E
+    n_copy: int = 0                #   router outputs, in this order; weights are held for the first E - n_zc experts
+    n_const: int = 0
+    aux_coef: float = 0.0          # auxiliary load-balancing loss coefficient; 0 = off
+    aux_zc_weight: float = 1.0     # weight of the zero-computation experts in the balance term
     # input recipe only (not part of moe_config_t)
     w_std: float = 0.02            # expert weight std; <0 means 1/sqrt(fan_in) (configs[0])
     bias_kind: str = "none"        # "none" | "normal" (b~N(0,0.05)) | "zipf" (configs[4] skew offset)
@@ -56,6 +63,11 @@ class MoEConfig:
     @property
     def TK(self) -> int:
         return self.T * self.K
+
+    @property
+    def E_ffn(self) -> int:
+        """Experts that own FFN weights (all of them unless zero-computation experts are configured)."""
+        return self.E - self.n_zero - self.n_copy - self.n_const
 
     @property
     def TK_pad(self) -> int:
@@ -195,16 +207,30 @@ def gen_shared_weights(cfg: MoEConfig):
 def gen_all_expert_weights(cfg: MoEConfig, threads: int = 8):
     """Stacked (Wg[E,F,H], Wu[E,F,H], Wd[E,H,F]) fp32 arrays; experts generated in parallel
     (each from its own stream, so the result does not depend on the thread count)."""
-    Wg = np.empty((cfg.E, cfg.F, cfg.H), np.float32)
-    Wu = np.empty((cfg.E, cfg.F, cfg.H), np.float32)
-    Wd = np.empty((cfg.E, cfg.H, cfg.F), np.float32)
+    Wg = np.empty((cfg.E_ffn, cfg.F, cfg.H), np.float32)
+    Wu = np.empty((cfg.E_ffn, cfg.F, cfg.H), np.float32)
+    Wd = np.empty((cfg.E_ffn, cfg.H, cfg.F), np.float32)
 
     def one(e):
         Wg[e], Wu[e], Wd[e] = gen_expert_weights(cfg, e)
 
     with ThreadPoolExecutor(max_workers=threads) as ex:
-        list(ex.map(one, range(cfg.E)))
+        list(ex.map(one, range(cfg.E_ffn)))
     return Wg, Wu, Wd
+
+
+def gen_threshold(cfg: MoEConfig) -> np.ndarray:
+    """Per-expert gate thresholds of the variable-k router (route_mode 1), fp32 in (0, 1): N(0.62, 0.03) so that with
+    logits of std 0.91 a token activates a handful of experts, some tokens none (top-1 fallback) and some more than K."""
+    t = 0.62 + normal(cfg.seed, "aux", (cfg.E,), 0.03, DTYPE_FP32, 1)
+    return np.clip(t, 0.05, 0.95).astype(np.float32)
+
+
+def gen_zc_const(cfg: MoEConfig):
+    """Constant experts' vectors [n_const, H] (activation dtype grid), or None."""
+    if cfg.n_const == 0:
+        return None
+    return normal(cfg.seed, "aux", (cfg.n_const, cfg.H), 1.0, _act_dtype(cfg), 2)
 
 
 def gen_logits(cfg: MoEConfig, std: float = 0.91, ties: int = 0) -> np.ndarray:
