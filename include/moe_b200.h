@@ -49,7 +49,26 @@ typedef struct moe_config_t {
   int32_t dtype;               /* 0 = fp32, 1 = bf16, 2 = fp8-e4m3 block-scaled GEMMs with bf16 I/O    */
   int32_t fp8_scale_mode;      /* 0 = fp32 amax/448, 1 = power of two (R9)                             */
   int32_t row_align;           /* expert groups start at multiples of this many rows (>= 1)            */
+  /* ---- widened rows; all zero = the plain top-k layer ---- */
+  int32_t route_mode;          /* 0 = top-k (R2..R5); 1 = threshold-gated variable-k on sigmoid gates (V1,
+                                  PAPER.md:456): needs score_fn = 1, n_group = 1, thresholds in moe_extras_t    */
+  int32_t n_zero, n_copy, n_const; /* zero-computation experts (V2): the LAST n_zero + n_copy +
+                                  n_const of the E router outputs, in this order; they own no FFN weights:
+                                  Wg, Wu, Wd and their gradients hold E - n_zero - n_copy - n_const experts    */
+  float aux_coef;              /* auxiliary load-balancing loss coefficient (A1); 0 = off    */
+  float aux_zc_weight;         /* weight of the zero-computation experts in the balance term    */
 } moe_config_t;
+
+/* Optional inputs / outputs of the widened rows, passed to moe_layer_fwd_ex / moe_layer_bwd_ex (NULL members that the
+ * config does not need are ignored).  All device pointers. */
+typedef struct moe_extras_t {
+  const float* threshold;    /* [E] fp32 gate thresholds, required iff route_mode == 1 (no gradient)              */
+  const void* zc_const;      /* [n_const, H] constant experts' vectors (activation type), required iff n_const > 0 */
+  void* d_zc_const;          /* bwd: [n_const, H] their gradient, overwritten; NULL = not wanted                   */
+  const float* aux_f_global; /* [E] fp32 or NULL: assignment fractions f_e of the GLOBAL batch (e.g. counts
+                                all-reduced over data-parallel ranks and normalised); NULL = this batch's own     */
+  float* aux_loss;           /* fwd: device scalar that receives L_aux, or NULL                                    */
+} moe_extras_t;
 
 enum moe_status {
   MOE_OK = 0,
@@ -82,6 +101,14 @@ int32_t moe_workspace_bytes(const moe_config_t* cfg, size_t* ws_bytes, size_t* c
  * UNSUPPORTED: E > 1024, K > 32, n_group > 32, K > topk_group * E / n_group. */
 int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
                   float* topk_w, void* stream);
+
+/* V1: threshold-gated variable-k routing.  s = sigmoid(z) (evaluated as in moe_route);
+ * expert e is active for a token iff s[e] > threshold[e]; the active experts fill the K slots in (s desc, index asc)
+ * order (more than K active: the K largest stay), unused slots hold topk_idx = -1 and topk_w = 0; a token no expert
+ * admits keeps its single best expert.  Weights: routed_scale * s_j / (sum of the selected s + 1e-20) (renorm) or
+ * routed_scale * s_j.  Every other entry point accepts the -1 slots (they own no permuted row). */
+int32_t moe_route_threshold(const moe_config_t* cfg, const float* logits, const float* threshold, int32_t* topk_idx,
+                            float* topk_w, void* stream);
 
 /* R6.  Histogram, exclusive scan, stable counting sort of flat positions
  * p = t*K + j by expert (no atomics; deterministic), then the row gather Xp[r] = X[perm_to_flat[r] / K].
@@ -152,6 +179,18 @@ int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const void* Wr, co
                       const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
                       void* stream);
 
+/* The forward with the widened rows' extras (`ex` may be NULL when the config needs none; moe_layer_fwd is this call
+ * with ex = NULL):  route_mode 1 routes with ex->threshold (V1);  zero-computation experts (V2) contribute
+ * w * 0 / w * X[t] / w * zc_const[c] and run no GEMM;  aux_coef != 0 (A1..A2) also computes
+ *   L_aux = aux_coef * E * sum_e eta_e f_e P_e,   f_e = fraction of the routed assignments on expert e (ex->aux_f_global
+ *   if given, else this batch's counts / assignments made),   P_e = mean over tokens of p[t,e]  (p = softmax(z) for
+ *   score_fn 0, s / sum_e s for sigmoid gates),   eta_e = aux_zc_weight for zero-computation experts, else 1,
+ * stores f in ctx for the backward and writes L_aux to ex->aux_loss (also readable as ctx field "aux_loss"). */
+int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
+                         const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                         const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
+                         const moe_extras_t* ex, void* stream);
+
 /* R8: the whole backward for L = <Y, dY>.  Weight gradients are overwritten, in the weights' type.
  * Any of dWr / dWg / dWu / dWd (and the shared triple) may be NULL together with the others of its
  * group to skip the weight-gradient GEMMs (dX is always produced).
@@ -161,6 +200,16 @@ int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const void* X, co
                       const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
                       const void* ctx, void* dX, void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s,
                       void* dWu_s, void* dWd_s, void* ws, void* stream);
+
+/* The backward with the extras: L = <Y, dY> + L_aux.  The balance term adds the dense gradient
+ *   dz[t,j] += (aux_coef E / T) d_j (g_j - sum_e g_e p[t,e]),  g = eta * f,  d_j = p_j (softmax) or s_j (1 - s_j) / sum_e s_e
+ * (A3; f carries no gradient) to the router backward, which then runs as two dense GEMMs (dWr = dz^T X, dX += dz Wr);
+ * the same dense path serves softmax gating without renormalisation.  ex->d_zc_const receives sum_r dy[r] per constant
+ * expert.  moe_layer_bwd is this call with ex = NULL. */
+int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, const void* X, const void* Wr, const void* Wg,
+                         const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
+                         const void* ctx, void* dX, void* dWr, void* dWg, void* dWu, void* dWd, void* dWg_s,
+                         void* dWu_s, void* dWd_s, void* ws, const moe_extras_t* ex, void* stream);
 
 /* R8, weight gradients only -- the separately schedulable half of the backward that a delayed weight-gradient
  * schedule needs (PAPER.md:116 "wgrad delay", :239).  Call moe_layer_bwd with NULL weight gradients first (dgrad, dX,
@@ -205,10 +254,11 @@ int32_t moe_layer_step_host_pipelined(void* pipeline, const moe_config_t* cfg, i
                                       void* stream_compute, void* stream_out);
 
 /* Read-only view of buffers inside ctx after moe_layer_fwd (for tests and tracing):
- * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s"}.
+ * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s",
+ *          "aux_f","aux_P","aux_loss" (fp32 [E], [E], [1]; aux_coef != 0)}.
  * Writes the byte offset inside ctx and the byte length.  */
 int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
-/* Same for ws after moe_layer_bwd: {"dw","dz","dy","dgu","dXp"}. */
+/* Same for ws after moe_layer_bwd: {"dw","dz","dy","dgu","dXp","dz_dense" (fp32 [T,E]; dense router backward only)}. */
 int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
 
 /* Stage timing for bench.py: while enabled, moe_layer_fwd / moe_layer_bwd record a CUDA event on

@@ -21,7 +21,14 @@ class moe_config_t(C.Structure):
                 ("n_group", C.c_int32), ("topk_group", C.c_int32), ("score_fn", C.c_int32),
                 ("group_score", C.c_int32), ("renorm", C.c_int32), ("routed_scale", C.c_float),
                 ("has_bias", C.c_int32), ("F_shared", C.c_int32), ("dtype", C.c_int32),
-                ("fp8_scale_mode", C.c_int32), ("row_align", C.c_int32)]
+                ("fp8_scale_mode", C.c_int32), ("row_align", C.c_int32),
+                ("route_mode", C.c_int32), ("n_zero", C.c_int32), ("n_copy", C.c_int32), ("n_const", C.c_int32),
+                ("aux_coef", C.c_float), ("aux_zc_weight", C.c_float)]
+
+
+class moe_extras_t(C.Structure):
+    _fields_ = [("threshold", C.c_void_p), ("zc_const", C.c_void_p), ("d_zc_const", C.c_void_p),
+                ("aux_f_global", C.c_void_p), ("aux_loss", C.c_void_p)]
 
 
 CONFIG_FIELDS = [f for f, _ in moe_config_t._fields_]
@@ -51,6 +58,9 @@ _SIGNATURES = {
     "moe_padded_rows": (_I64, [_CFG]),
     "moe_workspace_bytes": (_I32, [_CFG, _SZP, _SZP]),
     "moe_route": (_I32, [_CFG, _P, _P, _P, _P, _P]),
+    "moe_route_threshold": (_I32, [_CFG, _P, _P, _P, _P, _P]),
+    "moe_layer_fwd_ex": (_I32, [_CFG] + [_P] * 14 + [C.POINTER(moe_extras_t), _P]),
+    "moe_layer_bwd_ex": (_I32, [_CFG] + [_P] * 19 + [C.POINTER(moe_extras_t), _P]),
     "moe_permute": (_I32, [_CFG] + [_P] * 9),
     "moe_grouped_gemm_fwd": (_I32, [_CFG, _I32, _I32] + [_P] * 8),
     "moe_grouped_gemm_bwd": (_I32, [_CFG, _I32, _I32] + [_P] * 8),
@@ -174,6 +184,33 @@ def moe_ws_field(cfg, name):
 def moe_route(cfg, logits, bias, topk_idx, topk_w, stream=None):
     _check(lib().moe_route(C.byref(make_config(cfg)), _ptr(logits), _ptr(bias), _ptr(topk_idx), _ptr(topk_w),
                            _stream(stream)), "moe_route")
+
+
+def moe_route_threshold(cfg, logits, threshold, topk_idx, topk_w, stream=None):
+    _check(lib().moe_route_threshold(C.byref(make_config(cfg)), _ptr(logits), _ptr(threshold), _ptr(topk_idx),
+                                     _ptr(topk_w), _stream(stream)), "moe_route_threshold")
+
+
+def make_extras(threshold=None, zc_const=None, d_zc_const=None, aux_f_global=None, aux_loss=None) -> moe_extras_t:
+    """moe_extras_t from torch tensors (None = NULL)."""
+    def a(t):
+        return None if t is None else _ptr(t).value
+    return moe_extras_t(a(threshold), a(zc_const), a(d_zc_const), a(aux_f_global), a(aux_loss))
+
+
+def moe_layer_fwd_ex(cfg, X, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, Y, topk_idx, topk_w, ctx, ws, extras, stream=None):
+    _check(lib().moe_layer_fwd_ex(C.byref(make_config(cfg)), _ptr(X), _ptr(Wr), _ptr(bias), _ptr(Wg), _ptr(Wu), _ptr(Wd),
+                                  _ptr(Wg_s), _ptr(Wu_s), _ptr(Wd_s), _ptr(Y), _ptr(topk_idx), _ptr(topk_w), _ptr(ctx),
+                                  _ptr(ws), C.byref(extras) if extras is not None else None, _stream(stream)),
+           "moe_layer_fwd_ex")
+
+
+def moe_layer_bwd_ex(cfg, dY, X, Wr, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, dX, dWr, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, ws,
+                     extras, stream=None):
+    _check(lib().moe_layer_bwd_ex(C.byref(make_config(cfg)), _ptr(dY), _ptr(X), _ptr(Wr), _ptr(Wg), _ptr(Wu), _ptr(Wd),
+                                  _ptr(Wg_s), _ptr(Wu_s), _ptr(Wd_s), _ptr(ctx), _ptr(dX), _ptr(dWr), _ptr(dWg),
+                                  _ptr(dWu), _ptr(dWd), _ptr(dWg_s), _ptr(dWu_s), _ptr(dWd_s), _ptr(ws),
+                                  C.byref(extras) if extras is not None else None, _stream(stream)), "moe_layer_bwd_ex")
 
 
 def moe_permute(cfg, X, topk_idx, counts, offsets, perm_to_flat, flat_to_perm, Xp, ws, stream=None):

@@ -5,7 +5,8 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from . import (make_config, moe_ctx_field, moe_layer_bwd, moe_layer_fwd, moe_layer_step_host,
+from . import (make_config, make_extras, moe_ctx_field, moe_layer_bwd, moe_layer_bwd_ex, moe_layer_fwd, moe_layer_fwd_ex,
+               moe_layer_step_host,
                moe_layer_step_host_pipelined, moe_padded_rows, moe_pipeline_create, moe_pipeline_destroy,
                moe_workspace_bytes, moe_ws_field)
 
@@ -44,7 +45,8 @@ class LayerBuffers:
         self.X, self.dY, self.Y, self.dX = e(T, H), e(T, H), e(T, H), e(T, H)
         self.Wr = e(E, H)
         self.bias = e(E, dtype=torch.float32) if cfg.has_bias else None
-        self.Wg, self.Wu, self.Wd = e(E, F, H), e(E, F, H), e(E, H, F)
+        Ef = E - getattr(cfg, "n_zero", 0) - getattr(cfg, "n_copy", 0) - getattr(cfg, "n_const", 0)   # experts with FFN weights
+        self.Wg, self.Wu, self.Wd = e(Ef, F, H), e(Ef, F, H), e(Ef, H, F)
         self.Wg_s = self.Wu_s = self.Wd_s = None
         if Fs:
             self.Wg_s, self.Wu_s, self.Wd_s = e(Fs, H), e(Fs, H), e(H, Fs)
@@ -52,13 +54,26 @@ class LayerBuffers:
         self.topk_w = e(T, K, dtype=torch.float32)
         self.dWr = self.dWg = self.dWu = self.dWd = self.dWg_s = self.dWu_s = self.dWd_s = None
         if with_grads:
-            self.dWr, self.dWg, self.dWu, self.dWd = e(E, H), e(E, F, H), e(E, F, H), e(E, H, F)
+            self.dWr, self.dWg, self.dWu, self.dWd = e(E, H), e(Ef, F, H), e(Ef, F, H), e(Ef, H, F)
             if Fs:
                 self.dWg_s, self.dWu_s, self.dWd_s = e(Fs, H), e(Fs, H), e(H, Fs)
+        # extras of the widened rows (moe_extras_t): thresholds, constant experts, balance loss
+        self.threshold = e(E, dtype=torch.float32) if getattr(cfg, "route_mode", 0) == 1 else None
+        nc = getattr(cfg, "n_const", 0)
+        self.zc_const = e(nc, H) if nc else None
+        self.d_zc_const = e(nc, H) if (nc and with_grads) else None
+        self.aux_loss = e(1, dtype=torch.float32) if getattr(cfg, "aux_coef", 0.0) else None
+        self.aux_f_global = None
+        self.use_ex = any(t is not None for t in (self.threshold, self.zc_const, self.aux_loss))
 
     # ---- loading inputs (numpy fp32 on the storage grid) ----
-    def load(self, X=None, dY=None, Wr=None, bias=None, W=None, shared=None):
+    def extras(self):
+        return make_extras(self.threshold, self.zc_const, self.d_zc_const, self.aux_f_global, self.aux_loss)
+
+    def load(self, X=None, dY=None, Wr=None, bias=None, W=None, shared=None, threshold=None, zc_const=None):
         dt = act_dtype(self.cfg)
+        if threshold is not None: self.threshold.copy_(to_device(threshold, torch.float32, self.device))
+        if zc_const is not None: self.zc_const.copy_(to_device(zc_const, dt, self.device))
         if X is not None: self.X.copy_(to_device(X, dt, self.device))
         if dY is not None: self.dY.copy_(to_device(dY, dt, self.device))
         if Wr is not None: self.Wr.copy_(to_device(Wr, dt, self.device))
@@ -72,10 +87,17 @@ class LayerBuffers:
 
     # ---- the two calls ----
     def forward(self, stream=None):
+        if self.use_ex:
+            return moe_layer_fwd_ex(self.ccfg, self.X, self.Wr, self.bias, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s,
+                                    self.Wd_s, self.Y, self.topk_idx, self.topk_w, self.ctx, self.ws, self.extras(), stream)
         moe_layer_fwd(self.ccfg, self.X, self.Wr, self.bias, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s,
                       self.Wd_s, self.Y, self.topk_idx, self.topk_w, self.ctx, self.ws, stream)
 
     def backward(self, stream=None):
+        if self.use_ex:
+            return moe_layer_bwd_ex(self.ccfg, self.dY, self.X, self.Wr, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s,
+                                    self.Wd_s, self.ctx, self.dX, self.dWr, self.dWg, self.dWu, self.dWd, self.dWg_s,
+                                    self.dWu_s, self.dWd_s, self.ws, self.extras(), stream)
         moe_layer_bwd(self.ccfg, self.dY, self.X, self.Wr, self.Wg, self.Wu, self.Wd, self.Wg_s, self.Wu_s,
                       self.Wd_s, self.ctx, self.dX, self.dWr, self.dWg, self.dWu, self.dWd, self.dWg_s, self.dWu_s,
                       self.dWd_s, self.ws, stream)
@@ -112,10 +134,12 @@ class LayerBuffers:
             "flat_to_perm": ("i32", lambda c, R: (c.T * c.K,)), "Xp": ("act", lambda c, R: (R, c.H)),
             "gu": ("act", lambda c, R: (R, 2 * c.F)), "a": ("act", lambda c, R: (R, c.F)),
             "y": ("act", lambda c, R: (R, c.H)), "gu_s": ("act", lambda c, R: (c.T, 2 * c.F_shared)),
-            "a_s": ("act", lambda c, R: (c.T, c.F_shared)), "y_s": ("act", lambda c, R: (c.T, c.H))}
+            "a_s": ("act", lambda c, R: (c.T, c.F_shared)), "y_s": ("act", lambda c, R: (c.T, c.H)),
+            "aux_f": ("f32", lambda c, R: (c.E,)), "aux_P": ("f32", lambda c, R: (c.E,)),
+            "aux_loss": ("f32", lambda c, R: (1,))}
     _WS = {"dw": ("f32", lambda c, R: (c.T, c.K)), "dz": ("f32", lambda c, R: (c.T, c.K)),
            "dy": ("act", lambda c, R: (R, c.H)), "dgu": ("act", lambda c, R: (R, 2 * c.F)),
-           "dXp": ("act", lambda c, R: (R, c.H))}
+           "dXp": ("act", lambda c, R: (R, c.H)), "dz_dense": ("f32", lambda c, R: (c.T, c.E))}
 
     def _view(self, buf, field_fn, table, name):
         kind, shape_fn = table[name]

@@ -69,10 +69,20 @@ inline int64_t padded_rows(const moe_config_t* c) {
   return round_up(tk + (int64_t)c->E * (c->row_align - 1), c->row_align);
 }
 inline size_t elem_bytes(const moe_config_t* c) { return c->dtype == 0 ? 4 : 2; }
+// V2: zero-computation experts are the last n_zc of the E router outputs; the first E - n_zc own FFN weights.
+inline int n_zc(const moe_config_t* c) { return c->n_zero + c->n_copy + c->n_const; }
+inline int e_ffn(const moe_config_t* c) { return c->E - n_zc(c); }
+// The router backward runs densely (dz [T,E] -> two GEMMs) when dz is not confined to the selected experts: the balance
+// loss (A3), softmax gating without renormalisation; zero-computation experts use it too (their rows lie outside the
+// FFN tile tables the sparse dWr reduction walks).
+inline bool dense_router_bwd(const moe_config_t* c) {
+  return c->aux_coef != 0.f || n_zc(c) > 0 || (c->score_fn == 0 && !c->renorm && c->route_mode == 0);
+}
 
 // ---- byte layout of ctx / ws ---------------------------------------------------------------
 struct CtxLayout {
   size_t z, idx, w, counts, offsets, p2f, f2p, mtile, Xp, gu, a, y, gu_s, a_s, y_s;
+  size_t aux_f, aux_P, aux_loss;   // A1: fp32 [E], [E], [1]
   // fp8 (dtype 2): codes + scales of the quantised activations / weights kept for the backward
   size_t Xq, Xq_s, Xpq, Xpq_s, aq, aq_s, Wgq, Wgq_s, Wuq, Wuq_s, Wdq, Wdq_s;
   size_t asq, asq_s, Wgsq, Wgsq_s, Wusq, Wusq_s, Wdsq, Wdsq_s;
@@ -80,6 +90,7 @@ struct CtxLayout {
 };
 struct WsLayout {
   size_t hist, tmp, dw, dz, dzp, dwr_part, dy, dgu, dXp, dgu_s, dXs, dYq, dYq_s, dyq, dyq_s, dguq, dguq_s, dgusq, dgusq_s;
+  size_t dzd, dzb, dXr, aux_part;  // dense router backward: dz fp32 [T,E], its bf16 copy [T,Ep], dz Wr [T,H]; aux partials
   size_t total;
 };
 CtxLayout ctx_layout(const moe_config_t* c);
@@ -91,20 +102,33 @@ constexpr int PERM_CHUNK = 1024;  // flat positions per counting-sort chunk (one
 // permute.cu
 int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, int32_t* offsets, int32_t* p2f,
                    int32_t* f2p, int32_t* mtile_expert, int32_t* hist, cudaStream_t s);
+constexpr int AUX_TOKENS_PER_CTA = 64;   // tokens per partial sum of P_e (A2)
 int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, const int32_t* f2p, const int32_t* p2f,
                     const int32_t* offsets, void* Xp, cudaStream_t s);
 int32_t combine(const moe_config_t* c, const void* y, const float* w, const int32_t* f2p, const void* add0,
-                const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s);
+                const void* add1, const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s);
 int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const float* w, const int32_t* f2p,
                     const int32_t* p2f, const int32_t* offsets, void* dy, float* dw, cudaStream_t s);
 // route.cu: moe_route with an optional second copy of the outputs
-int32_t route_impl(const moe_config_t* c, const float* logits, const float* bias, int32_t* topk_idx, float* topk_w,
-                   int32_t* idx_copy, float* w_copy, void* stream);
+int32_t route_impl(const moe_config_t* c, const float* logits, const float* bias, const float* threshold,
+                   int32_t* topk_idx, float* topk_w, int32_t* idx_copy, float* w_copy, void* stream);
 // router.cu
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s);
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
                    const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const int32_t* mtile,
                    const void* Xp, float* dz, float* dzp, float* part, void* dWr, cudaStream_t s);
+// dense router backward (A3 / softmax without renorm / V2): dz [T,E] fp32 (+ bf16 copy), dWr = dz^T X, dXr = dz Wr
+int32_t router_bwd_dense(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
+                         const float* aux_f, const void* X, const void* Wr, const int32_t* off_one /* device {0, T} */,
+                         float* dz_sel, float* dzd, void* dzb, void* dWr, void* dXr, cudaStream_t s);
+// A1..A2: f (from counts, or f_global), P, L_aux -> ctx fields; loss also to loss_out if not NULL
+int32_t aux_forward(const moe_config_t* c, const float* z, const int32_t* counts, const float* f_global, float* part,
+                    float* aux_f, float* aux_P, float* aux_loss, float* loss_out, cudaStream_t s);
+// zc.cu (V2): rows of the zero-computation experts' groups
+int32_t zc_forward(const moe_config_t* c, const int32_t* offsets, const int32_t* counts, const void* Xp, const void* zc_const,
+                   void* gu, void* a, void* y, cudaStream_t s);
+int32_t zc_backward(const moe_config_t* c, const int32_t* offsets, const int32_t* counts, const void* dy, void* dgu, void* dXp,
+                    void* d_zc_const, cudaStream_t s);
 // gemm_simt.cu: reference-free fallback GEMMs for fp32 (and any shape the tensor-core path rejects)
 //   mode 0: C[r,n]    = sum_k A[r,k] B[e][n,k]           (rows grouped by offsets)
 //   mode 1: dA[r,k]   = sum_n dC[r,n] B[e][n,k]

@@ -214,7 +214,7 @@ extern "C" int32_t moe_fp8_quantize_weights(const moe_config_t* cfg, const void*
   if (shared && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
   cudaStream_t s = as_stream(stream);
   const CtxLayout C = ctx_layout(cfg);
-  const int m = cfg->fp8_scale_mode, E = cfg->E, H = cfg->H, F = cfg->F, Fs = cfg->F_shared;
+  const int m = cfg->fp8_scale_mode, E = e_ffn(cfg), H = cfg->H, F = cfg->F, Fs = cfg->F_shared;
   MOE_CHECK(fp8_quantize_weight(Wg, E, F, H, m, at<uint8_t>(ctx, C.Wgq), at<float>(ctx, C.Wgq_s), s));
   MOE_CHECK(fp8_quantize_weight(Wu, E, F, H, m, at<uint8_t>(ctx, C.Wuq), at<float>(ctx, C.Wuq_s), s));
   MOE_CHECK(fp8_quantize_weight(Wd, E, H, F, m, at<uint8_t>(ctx, C.Wdq), at<float>(ctx, C.Wdq_s), s));
@@ -230,9 +230,18 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
                                  const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
                                  const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
                                  void* stream) {
+  return moe_layer_fwd_ex(cfg, X, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, Y, topk_idx, topk_w, ctx, ws, nullptr, stream);
+}
+
+extern "C" int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, const void* Wr, const float* bias,
+                                    const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                                    const void* Wd_s, void* Y, int32_t* topk_idx, float* topk_w, void* ctx, void* ws,
+                                    const moe_extras_t* ex, void* stream) {
   if (!cfg || !X || !Wr || !Y || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(layer_preflight(cfg, false));
   if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
+  if (cfg->route_mode == 1 && !(ex && ex->threshold)) return MOE_ERR_INVALID_ARG;     // V1 needs the gate thresholds
+  if (cfg->n_const > 0 && !(ex && ex->zc_const)) return MOE_ERR_INVALID_ARG;          // V2 needs the constant vectors
   const bool shared = cfg->F_shared > 0;
   const bool fp8 = cfg->dtype == 2;
   // fp8: Wg == Wu == Wd == NULL means "use the e4m3 codes already in ctx" (the FP8 weight cache, PAPER.md:116,
@@ -258,13 +267,15 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
   prof_mark(ST_BEGIN, s);
   MOE_CHECK(router_logits(cfg, X, Wr, z, s));                                              // R1
   prof_mark(ST_ROUTER_GEMM, s);
-  MOE_CHECK(route_impl(cfg, z, bias, topk_idx, topk_w, at<int32_t>(ctx, C.idx), at<float>(ctx, C.w), stream));   // R2..R5
+  MOE_CHECK(route_impl(cfg, z, bias, ex ? ex->threshold : nullptr, topk_idx, topk_w, at<int32_t>(ctx, C.idx),
+                       at<float>(ctx, C.w), stream));                                                         // R2..R5 / V1
   prof_mark(ST_ROUTE, s);
   MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, p2f, f2p, mtile, at<int32_t>(ws, W.hist), s));  // R6
   prof_mark(ST_MAPS, s);
   MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, Xp, s));
   prof_mark(ST_PERMUTE, s);
-  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
+  // the FFN runs over the experts that own weights (all of them unless zero-computation experts are configured, V2)
+  FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
   Fp8Bufs q, qs;
@@ -295,10 +306,14 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
   } else {
     MOE_CHECK(ffn_fwd(g, Xp, Wg, Wu, Wd, gu, a, y, s));                                    // R7
   }
+  MOE_CHECK(zc_forward(cfg, offsets, counts, Xp, ex ? ex->zc_const : nullptr, gu, a, y, s));   // V2: y = 0 | x | v
+  if (cfg->aux_coef != 0.f)                                                                // A1..A2 balance loss
+    MOE_CHECK(aux_forward(cfg, z, counts, ex ? ex->aux_f_global : nullptr, at<float>(ws, W.aux_part), at<float>(ctx, C.aux_f),
+                          at<float>(ctx, C.aux_P), at<float>(ctx, C.aux_loss), ex ? ex->aux_loss : nullptr, s));
   const void* shared_out = nullptr;
+  if (shared || dense_router_bwd(cfg)) MOE_LAUNCH(set2_kernel, 1, 1, 0, s, offsets + cfg->E + 1, 0, cfg->T);   // group {0, T}
   if (shared) {
     int32_t* off_s = offsets + cfg->E + 1;
-    MOE_LAUNCH(set2_kernel, 1, 1, 0, s, off_s, 0, cfg->T);
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
     if (fp8)
@@ -307,7 +322,7 @@ extern "C" int32_t moe_layer_fwd(const moe_config_t* cfg, const void* X, const v
       MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
     shared_out = at<char>(ctx, C.y_s);
   }
-  MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, Y, s));    // R7 combine
+  MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, nullptr, Y, s));    // R7 combine
   prof_mark(ST_COMBINE, s);
   return MOE_OK;
 }
@@ -316,6 +331,15 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
                                  const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
                                  const void* Wd_s, const void* ctx, void* dX, void* dWr, void* dWg, void* dWu,
                                  void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, void* ws, void* stream) {
+  return moe_layer_bwd_ex(cfg, dY, X, Wr, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, ctx, dX, dWr, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, ws,
+                          nullptr, stream);
+}
+
+extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, const void* X, const void* Wr,
+                                    const void* Wg, const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s,
+                                    const void* Wd_s, const void* ctx, void* dX, void* dWr, void* dWg, void* dWu,
+                                    void* dWd, void* dWg_s, void* dWu_s, void* dWd_s, void* ws, const moe_extras_t* ex,
+                                    void* stream) {
   if (!cfg || !dY || !X || !Wr || !ctx || !dX || !ws) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(layer_preflight(cfg, true));
   const bool shared = cfg->F_shared > 0;
@@ -353,7 +377,7 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   prof_mark(ST_BEGIN, s);
   MOE_CHECK(combine_bwd(cfg, dY, y, w, f2p, p2f, offsets, dy, dw, s));                     // R8 combine-bwd
   prof_mark(ST_COMBINE_BWD, s);
-  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
+  FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
   Fp8Bufs q, qs;
@@ -384,8 +408,15 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
   } else {
     MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));     // R8 expert FFN
   }
-  MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr, Xp, dz,
-                       dzp, at<float>(ws, W.dwr_part), dWr, s));                                      // R8 router
+  MOE_CHECK(zc_backward(cfg, offsets, counts, dy, dgu, dXp, ex ? ex->d_zc_const : nullptr, s));      // V2: dXp = 0 | dy | 0
+  const bool dense = dense_router_bwd(cfg);
+  if (dense)                                                                                          // R8 router + A3
+    MOE_CHECK(router_bwd_dense(cfg, z, idx, w, dw, cfg->aux_coef != 0.f ? at<float>(ctx, C.aux_f) : nullptr, X, Wr,
+                               offsets + cfg->E + 1, dz, at<float>(ws, W.dzd), at<char>(ws, W.dzb), dWr, at<char>(ws, W.dXr),
+                               s));
+  else
+    MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr, Xp, dz,
+                         dzp, at<float>(ws, W.dwr_part), dWr, s));                                    // R8 router
   prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
   if (shared) {
@@ -400,8 +431,11 @@ extern "C" int32_t moe_layer_bwd(const moe_config_t* cfg, const void* dY, const 
                         at<char>(ws, W.dgu_s), at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
     dXs = at<char>(ws, W.dXs);
   }
-  // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]
-  MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, dz, idx, Wr, dX, s));
+  // dX[t] = sum_j dXp[f2p[tK+j]] + dXs[t] + sum_j dz[t,j] Wr[idx[t,j]]   (dense router backward: + (dz Wr)[t] instead)
+  if (dense)
+    MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, at<char>(ws, W.dXr), nullptr, nullptr, nullptr, dX, s));
+  else
+    MOE_CHECK(combine(cfg, dXp, nullptr, f2p, dXs, nullptr, dz, idx, Wr, dX, s));
   prof_mark(ST_DX_COMBINE, s);
   return MOE_OK;
 }
@@ -426,7 +460,7 @@ extern "C" int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const
   const CtxLayout C = ctx_layout(cfg);
   const WsLayout W = ws_layout(cfg);
   const int32_t* offsets = at<int32_t>(ctx, C.offsets);
-  FfnGroup g{cfg->dtype, cfg->E, cfg->H, cfg->F, padded_rows(cfg), offsets, at<int32_t>(ctx, C.counts),
+  FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, at<int32_t>(ctx, C.counts),
              (cfg->row_align % 128 == 0) ? at<int32_t>(ctx, C.mtile) : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
   prof_mark(ST_BEGIN, s);

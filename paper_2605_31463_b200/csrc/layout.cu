@@ -22,6 +22,11 @@ int32_t validate(const moe_config_t* c) {
   const int a = c->dtype == 0 ? 4 : 8;  // 16-byte rows
   if (c->H % a != 0 || c->F % a != 0 || c->F_shared % a != 0) return MOE_ERR_UNSUPPORTED;
   if (c->dtype == 2 && (c->H % 128 != 0 || c->F % 128 != 0 || c->F_shared % 128 != 0)) return MOE_ERR_UNSUPPORTED;
+  // widened rows
+  if (c->route_mode < 0 || c->route_mode > 1 || c->n_zero < 0 || c->n_copy < 0 || c->n_const < 0) return MOE_ERR_INVALID_ARG;
+  if (c->route_mode == 1 && (c->score_fn != 1 || c->n_group != 1 || c->has_bias)) return MOE_ERR_INVALID_ARG;
+  if (n_zc(c) >= c->E) return MOE_ERR_INVALID_ARG;              // at least one FFN expert
+  if (!(c->aux_coef == c->aux_coef) || !(c->aux_zc_weight == c->aux_zc_weight)) return MOE_ERR_INVALID_ARG;   // NaN
   return MOE_OK;
 }
 
@@ -80,6 +85,11 @@ CtxLayout ctx_layout(const moe_config_t* c) {
     L.a_s = k.take(T * Fs * es);
     L.y_s = k.take(T * H * es);
   }
+  if (c->aux_coef != 0.f) {
+    L.aux_f = k.take(E * 4);
+    L.aux_P = k.take(E * 4);
+    L.aux_loss = k.take(4);
+  }
   if (c->dtype == 2) {
     L.Xq = k.take(T * H); L.Xq_s = k.take(T * (H / 128) * 4);
     L.Xpq = k.take(R * H); L.Xpq_s = k.take(R * (H / 128) * 4);
@@ -128,6 +138,13 @@ WsLayout ws_layout(const moe_config_t* c) {
     L.dguq = k.take(R * 2 * F); L.dguq_s = k.take(R * (2 * F / 128) * 4);
     if (Fs) { L.dgusq = k.take(T * 2 * Fs); L.dgusq_s = k.take(T * (2 * Fs / 128) * 4); }
   }
+  if (dense_router_bwd(c)) {
+    const size_t Ep = (E + 63) / 64 * 64;       // bf16 copy padded so that it is a legal TMA / UMMA operand
+    L.dzd = k.take(T * E * 4);
+    L.dzb = k.take(T * Ep * 2);
+    L.dXr = k.take(T * H * es);
+  }
+  if (c->aux_coef != 0.f) L.aux_part = k.take(((T + AUX_TOKENS_PER_CTA - 1) / AUX_TOKENS_PER_CTA) * E * 4);
   L.total = k.cur;
   return L;
 }
@@ -173,11 +190,13 @@ extern "C" int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size
       {"z", L.z, T * E * 4}, {"counts", L.counts, E * 4}, {"offsets", L.offsets, (E + 1) * 4},
       {"perm_to_flat", L.p2f, R * 4}, {"flat_to_perm", L.f2p, T * cfg->K * 4}, {"Xp", L.Xp, R * H * es},
       {"gu", L.gu, R * 2 * F * es}, {"a", L.a, R * F * es}, {"y", L.y, R * H * es},
-      {"gu_s", L.gu_s, T * 2 * Fs * es}, {"a_s", L.a_s, T * Fs * es}, {"y_s", L.y_s, T * H * es}};
+      {"gu_s", L.gu_s, T * 2 * Fs * es}, {"a_s", L.a_s, T * Fs * es}, {"y_s", L.y_s, T * H * es},
+      {"aux_f", L.aux_f, E * 4}, {"aux_P", L.aux_P, E * 4}, {"aux_loss", L.aux_loss, 4}};
   for (auto& t : tab)
     if (strcmp(t.n, name) == 0) {
       const size_t nl = strlen(name);
       if (nl > 2 && strcmp(name + nl - 2, "_s") == 0 && !Fs) return MOE_ERR_INVALID_ARG;
+      if (strncmp(name, "aux_", 4) == 0 && cfg->aux_coef == 0.f) return MOE_ERR_INVALID_ARG;
       *byte_offset = t.off;
       *byte_len = t.len;
       return MOE_OK;
@@ -193,9 +212,10 @@ extern "C" int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_
   const size_t R = (size_t)padded_rows(cfg), T = cfg->T, H = cfg->H, F = cfg->F;
   struct { const char* n; size_t off, len; } tab[] = {
       {"dw", L.dw, T * cfg->K * 4}, {"dz", L.dz, T * cfg->K * 4}, {"dy", L.dy, R * H * es},
-      {"dgu", L.dgu, R * 2 * F * es}, {"dXp", L.dXp, R * H * es}};
+      {"dgu", L.dgu, R * 2 * F * es}, {"dXp", L.dXp, R * H * es}, {"dz_dense", L.dzd, T * (size_t)cfg->E * 4}};
   for (auto& t : tab)
     if (strcmp(t.n, name) == 0) {
+      if (strcmp(name, "dz_dense") == 0 && !dense_router_bwd(cfg)) return MOE_ERR_INVALID_ARG;
       *byte_offset = t.off;
       *byte_len = t.len;
       return MOE_OK;

@@ -19,7 +19,7 @@ __device__ __forceinline__ void warp_rank(const int32_t* __restrict__ idx, int64
 #pragma unroll
   for (int r = 0; r < CHUNK_ROUNDS; ++r) {
     const int64_t p = warp_base + r * 32 + lane;
-    const int e = (p < TK) ? idx[p] : -1;
+    const int e = (p < TK) ? idx[p] : -1;       // -1: past the end, or an empty slot of a variable-k router (V1)
     ex[r] = e;
     const unsigned m = __match_any_sync(FULL, e);
     const int before = __popc(m & ((1u << lane) - 1u));
@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(CHUNK_WARPS * 32) hist_kernel(const int32_t* _
 
 // Phase 2 (one CTA of 1024 threads): counts, aligned exclusive offsets, per-chunk bases (in place in
 // hist), and the tile tables of the tensor-core GEMMs (tile_tables.cuh) when row_align is a multiple of 128.
-__global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, int nchunks, int E, int row_align,
+__global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, int nchunks, int E, int E_tab, int row_align,
                                                     int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
                                                     int32_t* __restrict__ mtile, int32_t* __restrict__ plist,
                                                     int32_t* __restrict__ olist) {
@@ -77,7 +77,8 @@ __global__ void __launch_bounds__(1024) scan_kernel(int32_t* __restrict__ hist, 
       run += h;
     }
   }
-  if (mtile != nullptr) write_tile_tables(e, E, excl, incl, mtile, plist, olist, wsum);
+  // the GEMM tile tables cover the first E_tab experts (those that own FFN weights; V2: the rest compute nothing)
+  if (mtile != nullptr) write_tile_tables(e, E_tab, excl, incl, mtile, plist, olist, wsum);
 }
 
 // Phase 3: scatter.  flat_to_perm[p] = base[chunk][e] + rank of p among the chunk's positions of e.
@@ -111,6 +112,8 @@ __global__ void __launch_bounds__(CHUNK_WARPS * 32) scatter_kernel(const int32_t
       const int row = wh[warp * E + ex[r]] + rank[r];
       f2p[p] = row;
       p2f[row] = (int32_t)p;
+    } else if (p < TK) {
+      f2p[p] = -1;                                // an empty slot owns no permuted row
     }
   }
 }
@@ -127,7 +130,7 @@ int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, i
   MOE_LAUNCH(hist_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist);
   int32_t* mt = (c->row_align % 128 == 0) ? mtile_expert : nullptr;
   const int64_t R = padded_rows(c);
-  MOE_LAUNCH(scan_kernel, 1, 1024, 0, s, hist, nchunks, c->E, c->row_align, counts, offsets, mt,
+  MOE_LAUNCH(scan_kernel, 1, 1024, 0, s, hist, nchunks, c->E, e_ffn(c), c->row_align, counts, offsets, mt,
              mt ? mt + tile_plist_off(R) : nullptr, mt ? mt + tile_olist_off(R) : nullptr);
   MOE_LAUNCH(scatter_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist, p2f, f2p);
   return MOE_OK;

@@ -11,13 +11,14 @@ namespace {
 constexpr unsigned FULL = 0xffffffffu;
 
 struct RouteParams {
-  int T, E, K, n_group, topk_group, score_fn, group_score, renorm, has_bias;
+  int T, E, K, n_group, topk_group, score_fn, group_score, renorm, has_bias, route_mode;
   float routed_scale;
 };
 
 template <int VPT>
 __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* __restrict__ logits,
-                                                    const float* __restrict__ bias, int32_t* __restrict__ topk_idx,
+                                                    const float* __restrict__ bias,
+                                                    const float* __restrict__ threshold, int32_t* __restrict__ topk_idx,
                                                     float* __restrict__ topk_w, int32_t* __restrict__ idx_copy,
                                                     float* __restrict__ w_copy) {
   const int lane = threadIdx.x & 31;
@@ -94,6 +95,26 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
     }
   }
 
+  // ---- V1 threshold gating: only experts whose gate exceeds their threshold stay selectable; the
+  // number of filled slots is min(K, #active), or 1 (the best gate) when no expert admits the token ----
+  int n_fill = p.K;
+  if (p.route_mode == 1) {
+    int n_act = 0;
+    float masked[VPT];
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      const int e = s * 32 + lane;
+      const bool a = e < p.E && key[s] > threshold[e];
+      masked[s] = a ? key[s] : NEG;
+      n_act += __popc(__ballot_sync(FULL, a));
+    }
+    if (n_act > 0) {
+#pragma unroll
+      for (int s = 0; s < VPT; ++s) key[s] = masked[s];
+    }
+    n_fill = n_act == 0 ? 1 : min(n_act, p.K);
+  }
+
   // ---- R4 top-k: K rounds of arg-max, ties -> lower expert index ----
   // Keys are mapped to order-preserving unsigned integers (-0 folded into +0 first, so equal floats stay equal);
   // a round is two hardware warp reductions: redux.max of the lanes' best keys, then redux.min of the expert
@@ -126,8 +147,8 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
     if (lane == j) { sel_e = e; sel_z = zsel; }
   }
 
-  // ---- R5 gating weights (fp32) ----
-  const bool act = lane < p.K;
+  // ---- R5 gating weights (fp32); slots >= n_fill are empty (idx -1, weight 0) ----
+  const bool act = lane < n_fill;
   float wj;
   if (p.score_fn == 0) {
     float m, den;
@@ -161,7 +182,8 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
       wj = p.routed_scale * sj;
     }
   }
-  if (act) {
+  if (lane < p.K) {
+    if (!act) { sel_e = -1; wj = 0.f; }
     topk_idx[(size_t)t * p.K + lane] = sel_e;
     topk_w[(size_t)t * p.K + lane] = wj;
     if (idx_copy) {                                   // the copy moe_layer_fwd keeps in ctx for the backward
@@ -176,29 +198,37 @@ __global__ void __launch_bounds__(128) route_kernel(RouteParams p, const float* 
 }  // namespace moe
 
 namespace moe {
-int32_t route_impl(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx, float* topk_w,
-                   int32_t* idx_copy, float* w_copy, void* stream) {
+int32_t route_impl(const moe_config_t* cfg, const float* logits, const float* bias, const float* threshold,
+                   int32_t* topk_idx, float* topk_w, int32_t* idx_copy, float* w_copy, void* stream) {
   if (!cfg || !logits || !topk_idx || !topk_w) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(validate(cfg));
   if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
+  if (cfg->route_mode == 1 && !threshold) return MOE_ERR_INVALID_ARG;
   if (cfg->E > 1024 || cfg->K > 32 || cfg->n_group > 32) return MOE_ERR_UNSUPPORTED;
   RouteParams p{cfg->T, cfg->E, cfg->K, cfg->n_group, cfg->topk_group, cfg->score_fn, cfg->group_score,
-                cfg->renorm, cfg->has_bias, cfg->routed_scale};
+                cfg->renorm, cfg->has_bias, cfg->route_mode, cfg->routed_scale};
   const int warps = 4;
   dim3 grid((unsigned)ceil_div(cfg->T, warps)), block(warps * 32);
   cudaStream_t s = as_stream(stream);
   const int vpt = (int)ceil_div(cfg->E, 32);
-  if (vpt <= 1) MOE_LAUNCH(route_kernel<1>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
-  else if (vpt <= 2) MOE_LAUNCH(route_kernel<2>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
-  else if (vpt <= 4) MOE_LAUNCH(route_kernel<4>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
-  else if (vpt <= 8) MOE_LAUNCH(route_kernel<8>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
-  else if (vpt <= 16) MOE_LAUNCH(route_kernel<16>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
-  else MOE_LAUNCH(route_kernel<32>, grid, block, 0, s, p, logits, bias, topk_idx, topk_w, idx_copy, w_copy);
+  if (vpt <= 1) MOE_LAUNCH(route_kernel<1>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 2) MOE_LAUNCH(route_kernel<2>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 4) MOE_LAUNCH(route_kernel<4>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 8) MOE_LAUNCH(route_kernel<8>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
+  else if (vpt <= 16) MOE_LAUNCH(route_kernel<16>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
+  else MOE_LAUNCH(route_kernel<32>, grid, block, 0, s, p, logits, bias, threshold, topk_idx, topk_w, idx_copy, w_copy);
   return MOE_OK;
 }
 }  // namespace moe
 
 extern "C" int32_t moe_route(const moe_config_t* cfg, const float* logits, const float* bias, int32_t* topk_idx,
                              float* topk_w, void* stream) {
-  return moe::route_impl(cfg, logits, bias, topk_idx, topk_w, nullptr, nullptr, stream);
+  if (cfg && cfg->route_mode != 0) return MOE_ERR_INVALID_ARG;   // thresholds go through moe_route_threshold
+  return moe::route_impl(cfg, logits, bias, nullptr, topk_idx, topk_w, nullptr, nullptr, stream);
+}
+
+extern "C" int32_t moe_route_threshold(const moe_config_t* cfg, const float* logits, const float* threshold,
+                                       int32_t* topk_idx, float* topk_w, void* stream) {
+  if (!cfg || cfg->route_mode != 1 || !threshold) return MOE_ERR_INVALID_ARG;
+  return moe::route_impl(cfg, logits, nullptr, threshold, topk_idx, topk_w, nullptr, nullptr, stream);
 }

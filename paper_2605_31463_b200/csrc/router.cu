@@ -62,8 +62,8 @@ __global__ void __launch_bounds__(128) dz_kernel(const float* __restrict__ z, co
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * 4 + (threadIdx.x >> 5);
   if (t >= Tn) return;
-  const bool act = lane < K;
   const size_t p = (size_t)t * K + lane;
+  const bool act = lane < K && idx[p] >= 0;        // an empty slot (variable-k routing) has no gradient and no row
   const float wj = act ? w[p] : 0.f;
   const float dwj = act ? dw[p] : 0.f;
   float out;
@@ -93,6 +93,8 @@ __global__ void __launch_bounds__(128) dz_kernel(const float* __restrict__ z, co
   if (act) {
     dz[p] = out;
     dzp[f2p[p]] = out;
+  } else if (lane < K) {
+    dz[p] = 0.f;
   }
 }
 
@@ -181,7 +183,275 @@ __global__ void __launch_bounds__(256) dwr_reduce_kernel(const float* __restrict
   dWr[(size_t)e * H + h] = __float2bfloat16_rn(s);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// A1..A2 auxiliary load-balancing loss: P_e = mean_t p[t,e], f_e, L = coef E sum eta f P
+// ---------------------------------------------------------------------------------------------------------
+// p over ALL experts for one token held by a warp (lane l owns experts l, l+32, ...): softmax(z), or s / sum s for
+// sigmoid gates.  Also returns the per-lane derivative factor d_e with dp-ish meaning used by the backward:
+// softmax: d = p;  sigmoid: d = s (1 - s) / S.
+template <int VPT>
+__device__ __forceinline__ void token_probs(const float* __restrict__ zrow, int E, int lane, bool softmax, float (&p)[VPT],
+                                            float (&d)[VPT]) {
+  float zr[VPT];
+  float m = -INFINITY;
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) {
+    const int e = s * 32 + lane;
+    zr[s] = e < E ? zrow[e] : -INFINITY;
+    m = fmaxf(m, zr[s]);
+  }
+  float sum = 0.f;
+  if (softmax) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, off));
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      p[s] = (s * 32 + lane < E) ? expf(zr[s] - m) : 0.f;
+      sum += p[s];
+    }
+  } else {
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      p[s] = (s * 32 + lane < E) ? 1.0f / (1.0f + expf(-zr[s])) : 0.f;
+      sum += p[s];
+    }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(FULL, sum, off);
+  const float inv = 1.0f / sum;
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) {
+    const float raw = p[s];
+    p[s] = raw * inv;
+    d[s] = softmax ? p[s] : raw * (1.0f - raw) * inv;
+  }
+}
+
+// part[cta, e] = sum over the CTA's AUX_TOKENS_PER_CTA tokens of p[t, e]  (fixed order: warp w owns tokens w, w+8, ...;
+// the 8 warps' sums are added in warp order), so P is deterministic.
+template <int VPT>
+__global__ void __launch_bounds__(256) aux_part_kernel(const float* __restrict__ z, int Tn, int E, int softmax,
+                                                       float* __restrict__ part) {
+  extern __shared__ float red[];   // [8][E]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float acc[VPT];
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) acc[s] = 0.f;
+  const int t0 = blockIdx.x * AUX_TOKENS_PER_CTA;
+  for (int i = warp; i < AUX_TOKENS_PER_CTA; i += 8) {
+    const int t = t0 + i;
+    if (t >= Tn) break;
+    float p[VPT], d[VPT];
+    token_probs<VPT>(z + (size_t)t * E, E, lane, softmax != 0, p, d);
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) acc[s] += p[s];
+  }
+#pragma unroll
+  for (int s = 0; s < VPT; ++s)
+    if (s * 32 + lane < E) red[warp * E + s * 32 + lane] = acc[s];
+  __syncthreads();
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    float sum = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) sum += red[w * E + e];
+    part[(size_t)blockIdx.x * E + e] = sum;
+  }
+}
+
+// One CTA: P_e = (sum of the partials in CTA order) / T;  f_e = f_global[e] or counts[e] / sum counts;
+// L = coef * E * sum_e eta_e f_e P_e (summed in expert order by thread 0 after a fixed-order block reduction).
+__global__ void __launch_bounds__(1024) aux_final_kernel(const float* __restrict__ part, int nparts, int Tn, int E, int nzc,
+                                                         float coef, float zc_weight, const int32_t* __restrict__ counts,
+                                                         const float* __restrict__ f_global, float* __restrict__ aux_f,
+                                                         float* __restrict__ aux_P, float* __restrict__ aux_loss,
+                                                         float* __restrict__ loss_out) {
+  __shared__ float sh[1024];
+  __shared__ int total_sh;
+  const int e = threadIdx.x;
+  int cnt = (e < E && !f_global) ? counts[e] : 0;
+  // total assignments (integer, exact)
+  int v = cnt;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
+  __shared__ int wsum[32];
+  if ((e & 31) == 0) wsum[e >> 5] = v;
+  __syncthreads();
+  if (e == 0) {
+    int tot = 0;
+    for (int w = 0; w < 32; ++w) tot += wsum[w];
+    total_sh = tot;
+  }
+  __syncthreads();
+  float term = 0.f;
+  if (e < E) {
+    float P = 0.f;
+    for (int i = 0; i < nparts; ++i) P += part[(size_t)i * E + e];
+    P /= (float)Tn;
+    const float f = f_global ? f_global[e] : (float)cnt / (float)max(total_sh, 1);
+    aux_f[e] = f;
+    aux_P[e] = P;
+    term = (e >= E - nzc ? zc_weight : 1.0f) * f * P;
+  }
+  sh[e] = term;
+  __syncthreads();
+  if (e == 0) {
+    float sum = 0.f;
+    for (int i = 0; i < E; ++i) sum += sh[i];
+    const float L = coef * (float)E * sum;
+    aux_loss[0] = L;
+    if (loss_out) loss_out[0] = L;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// dense router backward: dz over ALL experts (A3, softmax without renormalisation, V2)
+// ---------------------------------------------------------------------------------------------------------
+// One warp per token.  dzd[t, :] (fp32) = main term (R8, confined to the selected experts except for softmax without
+// renorm) + balance term (A3);  dzb = its bf16 copy, row pitch Ep (zero beyond E);  dz_sel[t, j] = dzd[t, idx[t, j]].
+template <int VPT, typename TB>
+__global__ void __launch_bounds__(128) dz_dense_kernel(const float* __restrict__ z, const int32_t* __restrict__ idx,
+                                                       const float* __restrict__ w, const float* __restrict__ dw,
+                                                       const float* __restrict__ aux_f, int Tn, int E, int Ep, int K,
+                                                       int score_fn, int renorm, int route_mode, float c, float aux_c,
+                                                       int nzc, float zc_weight, float* __restrict__ dz_sel,
+                                                       float* __restrict__ dzd, TB* __restrict__ dzb) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (t >= Tn) return;
+  const bool softmax = score_fn == 0 && route_mode == 0;
+  float p[VPT], d[VPT], out[VPT];
+  token_probs<VPT>(z + (size_t)t * E, E, lane, softmax, p, d);
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) out[s] = 0.f;
+  // ---- A3: (coef E / T) d_e (g_e - sum_e' g_e' p_e'),  g = eta * f ----
+  if (aux_f != nullptr && aux_c != 0.f) {
+    float g[VPT], inner = 0.f;
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) {
+      const int e = s * 32 + lane;
+      g[s] = e < E ? (e >= E - nzc ? zc_weight : 1.0f) * aux_f[e] : 0.f;
+      inner += g[s] * p[s];
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) inner += __shfl_xor_sync(FULL, inner, off);
+#pragma unroll
+    for (int s = 0; s < VPT; ++s) out[s] = aux_c * d[s] * (g[s] - inner);
+  }
+  // ---- R8 main term on the selected experts (lane j < K holds slot j) ----
+  const size_t q = (size_t)t * K + lane;
+  const int ej = lane < K ? idx[q] : -1;
+  const bool act = ej >= 0;
+  const float wj = act ? w[q] : 0.f, dwj = act ? dw[q] : 0.f;
+  float val;
+  if (softmax) {
+    float inner = wj * dwj;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) inner += __shfl_xor_sync(FULL, inner, off);
+    if (renorm) {
+      val = (c != 0.f) ? wj * (dwj - inner / c) : 0.f;
+    } else {
+      val = wj * dwj;                                   // + the dense part -p_e * sum_i w_i dw_i below
+#pragma unroll
+      for (int s = 0; s < VPT; ++s) out[s] -= p[s] * inner;
+    }
+  } else {
+    const float zj = act ? z[(size_t)t * E + ej] : 0.f;
+    const float sj = act ? 1.0f / (1.0f + expf(-zj)) : 0.f;
+    float ds;
+    if (renorm) {
+      float S = sj, D = dwj * sj;
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        S += __shfl_xor_sync(FULL, S, off);
+        D += __shfl_xor_sync(FULL, D, off);
+      }
+      S += 1e-20f;
+      ds = c * (dwj / S - D / (S * S));
+    } else {
+      ds = c * dwj;
+    }
+    val = ds * sj * (1.0f - sj);
+  }
+  // scatter the K slot values to the lanes that own those experts (fixed slot order)
+  for (int j = 0; j < K; ++j) {
+    const int e = __shfl_sync(FULL, ej, j);
+    const float vj = __shfl_sync(FULL, val, j);
+    if (e < 0) continue;
+#pragma unroll
+    for (int s = 0; s < VPT; ++s)
+      if (s == (e >> 5) && lane == (e & 31)) out[s] += vj;
+  }
+  // gather the final values of the selected experts back to their slots
+  float mine = 0.f;
+  for (int j = 0; j < K; ++j) {
+    const int e = __shfl_sync(FULL, ej, j);
+    float vv = 0.f;
+#pragma unroll
+    for (int s = 0; s < VPT; ++s)
+      if (e >= 0 && s == (e >> 5)) vv = out[s];
+    vv = __shfl_sync(FULL, vv, e >= 0 ? (e & 31) : 0);
+    if (lane == j) mine = e >= 0 ? vv : 0.f;
+  }
+  if (lane < K) dz_sel[q] = mine;
+#pragma unroll
+  for (int s = 0; s < VPT; ++s) {
+    const int e = s * 32 + lane;
+    if (e < E) dzd[(size_t)t * E + e] = out[s];
+    if (dzb != nullptr && e < Ep) dzb[(size_t)t * Ep + e] = from_f<TB>(e < E ? out[s] : 0.f);
+  }
+}
+
 }  // namespace
+
+int32_t aux_forward(const moe_config_t* c, const float* z, const int32_t* counts, const float* f_global, float* part,
+                    float* aux_f, float* aux_P, float* aux_loss, float* loss_out, cudaStream_t s) {
+  if (c->E > 1024) return MOE_ERR_UNSUPPORTED;
+  const int nparts = (int)ceil_div(c->T, AUX_TOKENS_PER_CTA);
+  const int softmax = (c->score_fn == 0 && c->route_mode == 0) ? 1 : 0;
+  const size_t smem = (size_t)8 * c->E * sizeof(float);
+  const int vpt = (int)ceil_div(c->E, 32);
+#define MOE_AUX(V) MOE_LAUNCH(aux_part_kernel<V>, nparts, 256, smem, s, z, c->T, c->E, softmax, part)
+  if (vpt <= 1) MOE_AUX(1); else if (vpt <= 2) MOE_AUX(2); else if (vpt <= 4) MOE_AUX(4); else if (vpt <= 8) MOE_AUX(8);
+  else if (vpt <= 16) MOE_AUX(16); else MOE_AUX(32);
+#undef MOE_AUX
+  MOE_LAUNCH(aux_final_kernel, 1, 1024, 0, s, part, nparts, c->T, c->E, n_zc(c), c->aux_coef, c->aux_zc_weight, counts,
+             f_global, aux_f, aux_P, aux_loss, loss_out);
+  return MOE_OK;
+}
+
+int32_t router_bwd_dense(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
+                         const float* aux_f, const void* X, const void* Wr, const int32_t* off_one, float* dz_sel,
+                         float* dzd, void* dzb, void* dWr, void* dXr, cudaStream_t s) {
+  if (c->E > 1024 || c->K > 32) return MOE_ERR_UNSUPPORTED;
+  const int E = c->E, Ep = (E + 63) / 64 * 64, vpt = (int)ceil_div(Ep, 32);
+  const float aux_c = c->aux_coef * (float)E / (float)c->T;
+  const unsigned grid = (unsigned)ceil_div(c->T, 4);
+  const bool bf = c->dtype != 0;
+#define MOE_DZD(V)                                                                                                          do {                                                                                                                        if (bf) MOE_LAUNCH((dz_dense_kernel<V, __nv_bfloat16>), grid, 128, 0, s, z, idx, w, dw, aux_f, c->T, E, Ep, c->K,                             c->score_fn, c->renorm, c->route_mode, c->routed_scale, aux_c, n_zc(c), c->aux_zc_weight, dz_sel,                         dzd, (__nv_bfloat16*)dzb);                                                                             else MOE_LAUNCH((dz_dense_kernel<V, float>), grid, 128, 0, s, z, idx, w, dw, aux_f, c->T, E, Ep, c->K, c->score_fn,                        c->renorm, c->route_mode, c->routed_scale, aux_c, n_zc(c), c->aux_zc_weight, dz_sel, dzd,                                 (float*)nullptr);                                                                                       } while (0)
+  if (vpt <= 2) MOE_DZD(2); else if (vpt <= 4) MOE_DZD(4); else if (vpt <= 8) MOE_DZD(8); else if (vpt <= 16) MOE_DZD(16);
+  else MOE_DZD(32);
+#undef MOE_DZD
+  // dWr[e, h] = sum_t dz[t, e] X[t, h];  dXr[t, h] = sum_e dz[t, e] Wr[e, h]: one group of T rows
+  const bool tc = bf && c->H % 64 == 0 && E % 64 == 0;
+  if (tc) {
+    TcCall g;
+    if (dWr) {
+      memset(&g, 0, sizeof(g));
+      g.mode = TC_WGRAD; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.M = E; g.A2 = X; g.lda2 = c->H; g.N = c->H;
+      g.out0 = dWr; g.ld0 = c->H;
+      MOE_CHECK(tc_gemm(g, s));
+    }
+    memset(&g, 0, sizeof(g));
+    g.mode = TC_DGRAD; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.B0 = Wr; g.b_rows = E; g.b_cols = c->H;
+    g.N = c->H; g.out0 = dXr; g.ld0 = c->H;
+    return tc_gemm(g, s);
+  }
+  // CUDA-core path (fp32, or shapes the tensor-core kernels do not take): dz in the activation type, one group {0, T}
+  const void* dzc = bf ? (const void*)dzb : (const void*)dzd;
+  const int lddz = bf ? Ep : E;
+  if (dWr) MOE_CHECK(simt_grouped_gemm(2, c->dtype, 1, E, c->H, X, c->H, nullptr, dzc, lddz, off_one, dWr, 0, c->T, 0, s));
+  return simt_grouped_gemm(1, c->dtype, 1, E, c->H, nullptr, 0, Wr, dzc, lddz, off_one, dXr, c->H, c->T, 0, s);
+}
 
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s) {
   if (c->dtype != 0 && c->H % 64 == 0 && c->E % 4 == 0) {   // bf16: tcgen05 GEMM with fp32 output (one group of T rows)

@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
     }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
+      if (rows[j] < 0) continue;                    // empty slot (variable-k routing): no row
       int4* dst = Xp + (size_t)rows[j] * nvec;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
@@ -96,11 +97,13 @@ struct Vec<__nv_bfloat16> {
   }
 };
 
-// Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
+// Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t]) (+ add1[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
+// Empty slots (f2p = -1, variable-k routing) contribute nothing.
 template <typename T, int KT>
 __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
                                                                   const int32_t* __restrict__ f2p,
                                                                   const int4* __restrict__ add0,
+                                                                  const int4* __restrict__ add1,
                                                                   const float* __restrict__ dz,
                                                                   const int32_t* __restrict__ idx,
                                                                   const int4* __restrict__ Wr, int Tn, int Krt, int nvec,
@@ -118,7 +121,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
     if (KT > 0) {                       // all K row loads in flight before the first use
       int4 q[KT > 0 ? KT : 1];
 #pragma unroll
-      for (int j = 0; j < KT; ++j) q[j] = ldg_stream(y + (size_t)rows[j] * nvec + v);
+      for (int j = 0; j < KT; ++j) q[j] = rows[j] >= 0 ? ldg_stream(y + (size_t)rows[j] * nvec + v) : make_int4(0, 0, 0, 0);
 #pragma unroll
       for (int j = 0; j < KT; ++j) {
         const float wj = w ? w[(size_t)t * K + j] : 1.0f;
@@ -129,6 +132,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
       }
     } else {
       for (int j = 0; j < K; ++j) {
+        if (rows[j] < 0) continue;
         const float wj = w ? w[(size_t)t * K + j] : 1.0f;
         float f[N];
         Vec<T>::unpack(ldg_stream(y + (size_t)rows[j] * nvec + v), f);
@@ -142,11 +146,19 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
 #pragma unroll
       for (int i = 0; i < N; ++i) acc[i] += f[i];
     }
+    if (add1) {
+      float f[N];
+      Vec<T>::unpack(ldg_stream(add1 + (size_t)t * nvec + v), f);
+#pragma unroll
+      for (int i = 0; i < N; ++i) acc[i] += f[i];
+    }
     if (dz) {
       for (int j = 0; j < K; ++j) {
+        const int ej = idx[(size_t)t * K + j];
+        if (ej < 0) continue;
         const float d = dz[(size_t)t * K + j];
         float f[N];
-        Vec<T>::unpack(__ldg(Wr + (size_t)idx[(size_t)t * K + j] * nvec + v), f);
+        Vec<T>::unpack(__ldg(Wr + (size_t)ej * nvec + v), f);
 #pragma unroll
         for (int i = 0; i < N; ++i) acc[i] = fmaf(d, f[i], acc[i]);
       }
@@ -184,7 +196,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4*
       Vec<T>::unpack(ldg_stream(dY + (size_t)t * nvec + v), g);
       int4 q[KT > 0 ? KT : 1];
 #pragma unroll
-      for (int j = 0; j < KT; ++j) q[j] = ldg_stream(y + (size_t)r[j] * nvec + v);
+      for (int j = 0; j < KT; ++j) q[j] = r[j] >= 0 ? ldg_stream(y + (size_t)r[j] * nvec + v) : make_int4(0, 0, 0, 0);
 #pragma unroll
       for (int j = 0; j < KT; ++j) {
         float f[N], o[N];
@@ -194,7 +206,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4*
           dot[j] = fmaf(g[i], f[i], dot[j]);
           o[i] = wj[j] * g[i];
         }
-        stg_stream(dy + (size_t)r[j] * nvec + v, Vec<T>::pack(o));
+        if (r[j] >= 0) stg_stream(dy + (size_t)r[j] * nvec + v, Vec<T>::pack(o));   // empty slot: no row, dw = 0
       }
     }
 #pragma unroll
@@ -209,7 +221,7 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4*
       const int r = f2p[(size_t)t * K + j];
       const float wj = w[(size_t)t * K + j];
       float dot = 0.f;
-      for (int v = lane; v < nvec; v += 32) {
+      for (int v = lane; r >= 0 && v < nvec; v += 32) {
         float g[N], f[N], o[N];
         Vec<T>::unpack(__ldg(dY + (size_t)t * nvec + v), g);
         Vec<T>::unpack(ldg_stream(y + (size_t)r * nvec + v), f);
@@ -250,13 +262,13 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
 }
 
 int32_t combine(const moe_config_t* c, const void* y, const float* w, const int32_t* f2p, const void* add0,
-                const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s) {
+                const void* add1, const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s) {
   const size_t esz = elem_bytes(c);
   if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(c->H * esz / 16);
   const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
 #define MOE_COMBINE(TY, KT)                                                                                       \
-  MOE_LAUNCH((combine_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, dz, idx, \
+  MOE_LAUNCH((combine_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, (const int4*)add1, dz, idx, \
              (const int4*)Wr, c->T, c->K, nvec, (int4*)Y)
   if (c->dtype == 0) {
     MOE_COMBINE(float, 0);
@@ -321,5 +333,5 @@ extern "C" int32_t moe_unpermute_combine(const moe_config_t* cfg, const void* y,
   using namespace moe;
   if (!cfg || !y || !topk_w || !flat_to_perm || !Y) return MOE_ERR_INVALID_ARG;
   MOE_CHECK(validate(cfg));
-  return combine(cfg, y, topk_w, flat_to_perm, shared_out, nullptr, nullptr, nullptr, Y, as_stream(stream));
+  return combine(cfg, y, topk_w, flat_to_perm, shared_out, nullptr, nullptr, nullptr, nullptr, Y, as_stream(stream));
 }

@@ -30,17 +30,22 @@ def dump_routing_trace(out_dir: str, step_id: int, layers) -> str:
     return path
 
 
-def check_routing_trace(path: str, num_experts: int, weight_sum: float = 1.0, atol: float = 1e-4) -> int:
+def check_routing_trace(path: str, num_experts: int, weight_sum: float = 1.0, atol: float = 1e-4,
+                        variable_k: bool = False) -> int:
     """The programmatic check of PAPER.md:436 (App. B.2.2): IDs in [0, num_experts), gating weights non-negative and
-    summing to `weight_sum` (1, or the routed scaling factor) over the top-k of every token.  Returns the layer count."""
+    summing to `weight_sum` (1, or the routed scaling factor) over the top-k of every token.  `variable_k` (a
+    threshold-gated router): unused slots hold ID -1 with weight 0 and every token keeps >= 1 expert.
+    Returns the layer count."""
     z = np.load(path)
     n = 0
     while f"layer{n}.expert_ids" in z:
         idx, w = z[f"layer{n}.expert_ids"], z[f"layer{n}.gating_weights"]
         if idx.shape != w.shape:
             raise ValueError(f"layer {n}: shape mismatch")
-        if idx.min() < 0 or idx.max() >= num_experts:
+        if idx.min() < (-1 if variable_k else 0) or idx.max() >= num_experts:
             raise ValueError(f"layer {n}: expert ID out of range")
+        if variable_k and ((w[idx < 0] != 0).any() or (idx[:, 0] < 0).any()):
+            raise ValueError(f"layer {n}: an empty slot must have weight 0 and slot 0 must be filled")
         if (w < 0).any() or not np.allclose(w.sum(axis=1), weight_sum, atol=atol):
             raise ValueError(f"layer {n}: gating weights must be non-negative and sum to {weight_sum}")
         n += 1

@@ -54,7 +54,16 @@ def gen_inputs(cfg):
     X, dY, Wr, bias = wl.gen_X(cfg), wl.gen_dY(cfg), wl.gen_Wr(cfg), wl.gen_bias(cfg)
     W = wl.gen_all_expert_weights(cfg)
     shared = wl.gen_shared_weights(cfg)
-    return dict(X=X, dY=dY, Wr=Wr, bias=bias, W=W, shared=shared)
+    inp = dict(X=X, dY=dY, Wr=Wr, bias=bias, W=W, shared=shared)
+    if cfg.route_mode == 1:
+        inp["threshold"] = wl.gen_threshold(cfg)
+    if cfg.n_const:
+        inp["zc_const"] = wl.gen_zc_const(cfg)
+    return inp
+
+
+def oracle_extras(inp):
+    return {k: inp[k] for k in ("threshold", "zc_const", "f_global") if k in inp}
 
 
 def run_gpu_layer(cfg, inp, backward=True):
@@ -69,16 +78,22 @@ def run_gpu_layer(cfg, inp, backward=True):
     return lb
 
 
-def check_routing_replay(cfg, z_gpu, bias, idx_gpu, w_gpu, z_truth=None):
+def check_routing_replay(cfg, z_gpu, bias, idx_gpu, w_gpu, z_truth=None, threshold=None):
     """Bit-exact indices given identical logits (replay mode), fp32 weights within 1e-5; in truth mode a
-    mismatch is tolerated only at a verified near-tie of the fp64 keys (gap < 1e-5)."""
-    idx_o, w_o = orc.route(z_gpu, bias, cfg, key_dtype=np.float32)
+    mismatch is tolerated only at a verified near-tie of the fp64 keys (gap < 1e-5; threshold routing: also a gate
+    within 1e-5 of its threshold)."""
+    idx_o, w_o = orc.route(z_gpu, bias, cfg, key_dtype=np.float32, threshold=threshold)
     assert np.array_equal(idx_o, idx_gpu), f"routing indices differ on {(idx_o != idx_gpu).any(axis=1).sum()} tokens"
     assert orc.rel_fro(w_gpu, w_o) <= TOL_ROUTER
     if z_truth is not None:
-        idx_t, _ = orc.route(z_truth, bias, cfg)
+        idx_t, _ = orc.route(z_truth, bias, cfg, threshold=threshold)
         bad = np.nonzero((idx_t != idx_gpu).any(axis=1))[0]
-        if bad.size:
+        if bad.size and cfg.route_mode == 1:
+            s = orc.sigmoid(z_truth[bad])
+            srt = -np.sort(-s, axis=1)
+            gaps = np.minimum(np.abs(np.diff(srt, axis=1)).min(axis=1), np.abs(s - threshold[None, :].astype(np.float64)).min(axis=1))
+            assert (gaps < 1e-5).all(), f"truth-mode mismatch at a non-tie: min gaps {gaps}"
+        elif bad.size:
             key = orc.group_limit(orc.selection_keys(z_truth[bad], bias, cfg), cfg)
             srt = -np.sort(-key, axis=1)
             gaps = np.abs(np.diff(srt[:, :cfg.K + 1], axis=1)).min(axis=1)
@@ -96,8 +111,9 @@ def compare_layer(cfg, inp, lb, backward=True, tol=None):
     w_gpu = to_numpy(lb.topk_w)
     z_o = orc.router_logits(inp["X"], inp["Wr"])
     assert orc.rel_fro(z_gpu, z_o) <= TOL_ROUTER, f"router logits {orc.rel_fro(z_gpu, z_o)}"
-    n_near = check_routing_replay(cfg, z_gpu, inp["bias"], idx_gpu, w_gpu, z_truth=z_o)
-    fwd = orc.layer_fwd(cfg, inp["X"], inp["Wr"], inp["bias"], inp["W"], inp["shared"], forced_idx=idx_gpu)
+    n_near = check_routing_replay(cfg, z_gpu, inp["bias"], idx_gpu, w_gpu, z_truth=z_o, threshold=inp.get("threshold"))
+    ex = oracle_extras(inp)
+    fwd = orc.layer_fwd(cfg, inp["X"], inp["Wr"], inp["bias"], inp["W"], inp["shared"], forced_idx=idx_gpu, extras=ex)
     errs = {"near_ties": n_near}
     # integer maps: bit-exact
     for name, ref in (("counts", fwd["counts"]), ("offsets", fwd["offsets"]), ("flat_to_perm", fwd["flat_to_perm"])):
@@ -112,18 +128,29 @@ def compare_layer(cfg, inp, lb, backward=True, tol=None):
     acts = [("g", gu[:, :cfg.F], fwd["g"]), ("u", gu[:, cfg.F:], fwd["u"]),
             ("a", to_numpy(lb.ctx_view("a"))[:R], fwd["a"]), ("y", to_numpy(lb.ctx_view("y"))[:R], fwd["y"]),
             ("Y", to_numpy(lb.Y), fwd["Y"])]
+    if cfg.aux_coef:                                             # A1..A2: loss value, f, P (fp32 router-side quantities)
+        errs["aux_loss"] = abs(float(to_numpy(lb.aux_loss)[0]) - fwd["aux_loss"]) / abs(fwd["aux_loss"])
+        assert errs["aux_loss"] <= TOL_ROUTER, errs["aux_loss"]
+        assert float(to_numpy(lb.ctx_view("aux_loss"))[0]) == float(to_numpy(lb.aux_loss)[0])
+        assert orc.rel_fro(to_numpy(lb.ctx_view("aux_f")), fwd["aux_f"]) <= TOL_ROUTER
+        assert orc.rel_fro(to_numpy(lb.ctx_view("aux_P")), fwd["aux_P"]) <= TOL_ROUTER
+        del errs["aux_loss"]
     if backward:
-        bwd = orc.layer_bwd(cfg, inp["dY"], inp["X"], inp["Wr"], inp["W"], fwd, inp["shared"])
+        bwd = orc.layer_bwd(cfg, inp["dY"], inp["X"], inp["Wr"], inp["W"], fwd, inp["shared"], extras=ex)
         errs["dw"] = orc.rel_fro(to_numpy(lb.ws_view("dw")), bwd["dw"])
         errs["dWr"] = orc.rel_fro(to_numpy(lb.dWr), bwd["dWr"])
         dgu = to_numpy(lb.ws_view("dgu"))[:R]
         acts += [("dg", dgu[:, :cfg.F], bwd["dg"]), ("du", dgu[:, cfg.F:], bwd["du"]),
                  ("dXp", to_numpy(lb.ws_view("dXp"))[:R], bwd["dXp"]), ("dX", to_numpy(lb.dX), bwd["dX"])]
-        dz_sel = np.take_along_axis(bwd["dz"], idx_gpu.astype(np.int64), axis=1)
+        dz_sel = np.where(idx_gpu >= 0, np.take_along_axis(bwd["dz"], np.maximum(idx_gpu, 0).astype(np.int64), axis=1), 0.0)
         errs["dz"] = orc.rel_fro(to_numpy(lb.ws_view("dz")), dz_sel)
+        if cfg.aux_coef or cfg.n_zero + cfg.n_copy + cfg.n_const or (cfg.score_fn == 0 and not cfg.renorm and cfg.route_mode == 0):
+            errs["dz_dense"] = orc.rel_fro(to_numpy(lb.ws_view("dz_dense")), bwd["dz"])   # dense router backward (A3)
+        if cfg.n_const:
+            errs["dzc_const"] = orc.rel_fro(to_numpy(lb.d_zc_const), bwd["dzc_const"])
         for name, got in (("dWg", lb.dWg), ("dWu", lb.dWu), ("dWd", lb.dWd)):
             g = to_numpy(got)
-            per = [orc.rel_fro(g[e], bwd[name][e]) for e in range(cfg.E)]
+            per = [orc.rel_fro(g[e], bwd[name][e]) for e in range(cfg.E_ffn)]
             errs[name] = float(np.max(per))                      # S19: max over experts; empty expert -> exact 0
         if inp["shared"] is not None:
             for name, got in (("dWg_s", lb.dWg_s), ("dWu_s", lb.dWu_s), ("dWd_s", lb.dWd_s)):
