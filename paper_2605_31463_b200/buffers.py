@@ -136,15 +136,17 @@ class LayerBuffers:
             "y": ("act", lambda c, R: (R, c.H)), "gu_s": ("act", lambda c, R: (c.T, 2 * c.F_shared)),
             "a_s": ("act", lambda c, R: (c.T, c.F_shared)), "y_s": ("act", lambda c, R: (c.T, c.H)),
             "aux_f": ("f32", lambda c, R: (c.E,)), "aux_P": ("f32", lambda c, R: (c.E,)),
-            "aux_loss": ("f32", lambda c, R: (1,))}
+            "aux_loss": ("f32", lambda c, R: (1,)),
+            "aq": ("u8", lambda c, R: (R, c.F)), "aq_s": ("f32", lambda c, R: (R, c.F // 128))}
     _WS = {"dw": ("f32", lambda c, R: (c.T, c.K)), "dz": ("f32", lambda c, R: (c.T, c.K)),
            "dy": ("act", lambda c, R: (R, c.H)), "dgu": ("act", lambda c, R: (R, 2 * c.F)),
-           "dXp": ("act", lambda c, R: (R, c.H)), "dz_dense": ("f32", lambda c, R: (c.T, c.E))}
+           "dXp": ("act", lambda c, R: (R, c.H)), "dz_dense": ("f32", lambda c, R: (c.T, c.E)),
+           "dguq": ("u8", lambda c, R: (R, 2 * c.F)), "dguq_s": ("f32", lambda c, R: (R, 2 * c.F // 128))}
 
     def _view(self, buf, field_fn, table, name):
         kind, shape_fn = table[name]
         off, ln = field_fn(self.ccfg, name)
-        dt = {"f32": torch.float32, "i32": torch.int32, "act": act_dtype(self.cfg)}[kind]
+        dt = {"f32": torch.float32, "i32": torch.int32, "u8": torch.uint8, "act": act_dtype(self.cfg)}[kind]
         return buf[off:off + ln].view(dt).view(*shape_fn(self.cfg, self.R))
 
     def ctx_view(self, name):

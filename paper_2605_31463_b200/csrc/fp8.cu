@@ -4,7 +4,6 @@
 //  * the fp8 grouped GEMM: tcgen05 kind::f8f6f4 on TMA-fed 128x128x128 tiles; every 128-deep k-block's partial
 //    product lands in its own TMEM buffer and is promoted into fp32 register accumulators with the block scales
 //    (sa[row, kb] * sb[n-block, kb]) by eight epilogue warps -- the dequantisation is fused into the main loop.
-#include <cuda_fp8.h>
 #include <string.h>
 
 #include <algorithm>
@@ -20,22 +19,9 @@ constexpr unsigned FULL = 0xffffffffu;
 // ---------------------------------------------------------------------------------------------
 // quantisers
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ float block_scale(float amax, int mode) {
-  if (amax == 0.f) return 1.f;
-  float r = __fdiv_rn(amax, 448.0f);
-  if (mode == 1) {                       // 2^ceil(log2 r): r = m 2^ex, m in [0.5, 1)
-    int ex;
-    const float m = frexpf(r, &ex);
-    r = ldexpf(1.0f, m == 0.5f ? ex - 1 : ex);
-  }
-  return r;
-}
-
+__device__ __forceinline__ float block_scale(float amax, int mode) { return fp8_block_scale(amax, mode); }
 __device__ __forceinline__ uint32_t encode4(float a, float b, float c, float d, float scale) {
-  // cvt.rn.satfinite.e4m3x2.f32 packs two codes per instruction (.x -> low byte)
-  const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(a, scale), __fdiv_rn(b, scale)), __NV_SATFINITE, __NV_E4M3);
-  const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(__fdiv_rn(c, scale), __fdiv_rn(d, scale)), __NV_SATFINITE, __NV_E4M3);
-  return lo | (hi << 16);
+  return fp8_encode4(a, b, c, d, scale);
 }
 
 __device__ __forceinline__ void unpack8(const uint4& v, float (&f)[8]) {

@@ -21,7 +21,8 @@ constexpr int BM = 128, BN = 128, BK = 128, UK = 32;
 constexpr int STAGES = 6;
 constexpr int A_BYTES = BM * BK, B_BYTES = BN * BK, STAGE_BYTES = A_BYTES + B_BYTES;   // 16 + 16 KB
 constexpr int NBUF = 4;                                                                  // TMEM partial-product ring
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int XCH_BYTES = 2 * 2 * BM * 2 * 4;   // amax exchange of the fused quantisers: [parity][g|u][row][column half] fp32
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + XCH_BYTES + 1024 + 256;
 constexpr int EPI_WARPS = 8;
 constexpr int NTHREADS = 64 + EPI_WARPS * 32;
 constexpr int TMEM_COLS = NBUF * BN;   // 512
@@ -54,14 +55,27 @@ struct F8Params {
   int64_t ldgu;
   const int32_t* p2f;
   const float* w;
+  uint8_t* q_codes;         // fused Q-a / Q-dgu output (nullptr: not fused)
+  float* q_scales;
+  int q_mode;
 };
 
 struct Tile {
   int e, m0, n0;
 };
 
+// i = sequence number of the tile inside this CTA's persistent loop.  F8_FWD_SWIGLU walks the 64-column n-tiles in
+// PAIRS (i = 2q, 2q+1 are the two halves of one 128-column block of `a` on the SAME CTA), so that the fused Q-a sees a
+// whole 1x128 quantisation block; the other modes take one tile per step.
 template <int MODE>
-__device__ __forceinline__ bool decode_tile(const F8Params& p, int64_t t, int64_t total, Tile& tl) {
+__device__ __forceinline__ bool decode_tile(const F8Params& p, int64_t i, int64_t total, Tile& tl) {
+  int64_t t;
+  if (MODE == F8_FWD_SWIGLU) {
+    const int64_t unit = blockIdx.x + (i >> 1) * (int64_t)gridDim.x;    // (M-tile, n-pair)
+    t = unit * 2 + (i & 1);
+  } else {
+    t = blockIdx.x + i * (int64_t)gridDim.x;
+  }
   if (t >= total) return false;
   const int mt = (int)(t / p.n_tiles);
   tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == F8_FWD_SWIGLU ? BN / 2 : BN);
@@ -104,6 +118,11 @@ __device__ __forceinline__ uint4 pack8(const float* v) {
 
 __device__ __forceinline__ float fast_sigmoid8(float x) { return 1.0f / (1.0f + __expf(-x)); }
 
+// four e4m3 codes of v / scale (R9): IEEE division for fp32 scales, an exact multiplication for power-of-two scales
+__device__ __forceinline__ uint32_t enc4(float a, float b, float c, float d, float scale, float inv, int mode) {
+  return mode == 1 ? fp8_encode4_pow2(a, b, c, d, inv) : fp8_encode4(a, b, c, d, scale);
+}
+
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
@@ -114,7 +133,8 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   constexpr bool B_MN = (MODE == F8_DGRAD || MODE == F8_DGRAD_SWIGLU);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bars = base + STAGES * STAGE_BYTES;
+  float* const xch = reinterpret_cast<float*>(smem_raw + (base - smem_u32(smem_raw)) + STAGES * STAGE_BYTES);
+  const uint32_t bars = base + STAGES * STAGE_BYTES + XCH_BYTES;
   const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, pfull0 = bars + 16 * STAGES, pempty0 = pfull0 + 8 * NBUF;
   const uint32_t tmem_slot = pempty0 + 8 * NBUF;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -148,7 +168,7 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       int stage = 0;
       uint32_t phase = 0;
       Tile tl;
-      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      for (int64_t t = 0; decode_tile<MODE>(p, t, total, tl); ++t) {
         for (int kb = 0; kb < p.nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, phase ^ 1);
           const uint32_t fb = full0 + 8 * stage;
@@ -176,7 +196,7 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       int stage = 0, buf = 0;
       uint32_t phase = 0, bphase = 0;
       Tile tl;
-      for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+      for (int64_t t = 0; decode_tile<MODE>(p, t, total, tl); ++t) {
         for (int kb = 0; kb < p.nkb; ++kb) {
           mbar_wait(pempty0 + 8 * buf, bphase ^ 1);
           mbar_wait(full0 + 8 * stage, phase);
@@ -205,8 +225,9 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int c1 = (MODE == F8_FWD_SWIGLU) ? 64 + ch * 32 : ch * 64 + 32;
     int buf = 0;
     uint32_t bphase = 0;
+    float amax_prev = 0.f;                     // fused Q-a: |a| max of this thread's 32 columns in the pair's first half
     Tile tl;
-    for (int64_t t = blockIdx.x; decode_tile<MODE>(p, t, total, tl); t += gridDim.x) {
+    for (int64_t t = 0; decode_tile<MODE>(p, t, total, tl); ++t) {
       const int64_t row = (int64_t)tl.m0 + row_in_tile;
       const bool row_ok = row < p.rows_valid;
       const float* sa_row = p.a_scales + (row_ok ? row : 0) * p.a_nblk;
@@ -238,35 +259,87 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         if (++buf == NBUF) { buf = 0; bphase ^= 1; }
       }
-      if (!row_ok) {
-        // rows past the buffer: nothing to store
-      } else if (MODE == F8_FWD || MODE == F8_DGRAD) {
+      // rows past the buffer (row_ok false) store nothing, but still take part in the fused quantisers' barriers
+      if (MODE == F8_FWD || MODE == F8_DGRAD) {
         __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0;
+        if (row_ok) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          *reinterpret_cast<uint4*>(dst + c0 + q * 8) = pack8(acc0 + q * 8);
-          *reinterpret_cast<uint4*>(dst + c1 + q * 8) = pack8(acc1 + q * 8);
+          for (int q = 0; q < 4; ++q) {
+            *reinterpret_cast<uint4*>(dst + c0 + q * 8) = pack8(acc0 + q * 8);
+            *reinterpret_cast<uint4*>(dst + c1 + q * 8) = pack8(acc1 + q * 8);
+          }
         }
       } else if (MODE == F8_FWD_SWIGLU) {
         const int col = tl.n0 + ch * 32;
         __nv_bfloat16* gdst = p.out0 + row * p.ld0 + col;
         __nv_bfloat16* udst = gdst + p.F;
         __nv_bfloat16* adst = p.out1 + row * p.ld1 + col;
+        if (row_ok) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          *reinterpret_cast<uint4*>(gdst + q * 8) = pack8(acc0 + q * 8);
-          *reinterpret_cast<uint4*>(udst + q * 8) = pack8(acc1 + q * 8);
+          for (int q = 0; q < 4; ++q) {
+            *reinterpret_cast<uint4*>(gdst + q * 8) = pack8(acc0 + q * 8);
+            *reinterpret_cast<uint4*>(udst + q * 8) = pack8(acc1 + q * 8);
+          }
         }
 #pragma unroll
         for (int i = 0; i < 32; ++i) acc0[i] = acc0[i] * fast_sigmoid8(acc0[i]) * acc1[i];
+        uint4 ab[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) *reinterpret_cast<uint4*>(adst + q * 8) = pack8(acc0 + q * 8);
-      } else {  // F8_DGRAD_SWIGLU
+        for (int q = 0; q < 4; ++q) {
+          ab[q] = pack8(acc0 + q * 8);
+          if (row_ok) *reinterpret_cast<uint4*>(adst + q * 8) = ab[q];
+        }
+        if (p.q_codes) {
+          // fused Q-a (R9): quantise the bf16 a just written, 1 x 128 along F.  A block = the two 64-column halves this
+          // CTA computes back to back (t even, odd) x the two column-half warps of this lane group.
+          float am = 0.f;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint32_t wv[4] = {ab[q].x, ab[q].y, ab[q].z, ab[q].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) am = fmaxf(am, fmaxf(fabsf(bf16_lo(wv[i])), fabsf(bf16_hi(wv[i]))));
+          }
+          if ((t & 1) == 0) {
+            amax_prev = am;                                            // first half: wait for the second
+          } else {
+            am = fmaxf(am, amax_prev);
+            float* slot = xch + (((t >> 1) & 1) * 2 * BM + row_in_tile) * 2;
+            slot[ch] = am;
+            named_bar_sync(1 + lg, 64);                                // the two warps that share these 128 rows' blocks
+            const float sc = fp8_block_scale(fmaxf(slot[0], slot[1]), p.q_mode);
+            const float isc = 1.0f / sc;
+            if (row_ok) {
+            const int blk0 = tl.n0 - BN / 2;                           // first column of the 128-column block
+            uint8_t* cdst = p.q_codes + row * (int64_t)p.F + blk0 + ch * 32;
+            // first half: this thread's own earlier bf16 stores, read back (L2-hot, same thread: program order)
+            const volatile uint4* prev = reinterpret_cast<const volatile uint4*>(adst - BN / 2);
+            uint32_t c0w[8], c1w[8];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              uint4 pv;
+              pv.x = prev[q].x; pv.y = prev[q].y; pv.z = prev[q].z; pv.w = prev[q].w;
+              const uint32_t w0[4] = {pv.x, pv.y, pv.z, pv.w}, w1[4] = {ab[q].x, ab[q].y, ab[q].z, ab[q].w};
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                c0w[q * 2 + h] = enc4(bf16_lo(w0[2 * h]), bf16_hi(w0[2 * h]), bf16_lo(w0[2 * h + 1]), bf16_hi(w0[2 * h + 1]), sc, isc, p.q_mode);
+                c1w[q * 2 + h] = enc4(bf16_lo(w1[2 * h]), bf16_hi(w1[2 * h]), bf16_lo(w1[2 * h + 1]), bf16_hi(w1[2 * h + 1]), sc, isc, p.q_mode);
+              }
+            }
+            *reinterpret_cast<uint4*>(cdst) = make_uint4(c0w[0], c0w[1], c0w[2], c0w[3]);
+            *reinterpret_cast<uint4*>(cdst + 16) = make_uint4(c0w[4], c0w[5], c0w[6], c0w[7]);
+            *reinterpret_cast<uint4*>(cdst + BN / 2) = make_uint4(c1w[0], c1w[1], c1w[2], c1w[3]);
+            *reinterpret_cast<uint4*>(cdst + BN / 2 + 16) = make_uint4(c1w[4], c1w[5], c1w[6], c1w[7]);
+            if (ch == 0) p.q_scales[row * (int64_t)(p.F / 128) + blk0 / 128] = sc;
+            }
+          }
+        }
+      } else {  // F8_DGRAD_SWIGLU: this thread owns the 64 columns [ch * 64, ch * 64 + 64) of dg and of du of its row
         float rw = 1.0f;
-        if (p.w) {
+        if (p.w && row_ok) {
           const int pf = p.p2f[row];
           rw = pf >= 0 ? p.w[pf] : 0.f;
         }
+        uint4 dgp[8], dup[8];               // bf16 dg / du, 8 columns per uint4 (kept for the fused quantiser)
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
           const int col = tl.n0 + (half ? c1 : c0);
@@ -275,8 +348,11 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + col;
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
-            const uint4 gq = *reinterpret_cast<const uint4*>(gsrc + q * 8);
-            const uint4 uq = *reinterpret_cast<const uint4*>(gsrc + p.F + q * 8);
+            uint4 gq = make_uint4(0u, 0u, 0u, 0u), uq = gq;
+            if (row_ok) {
+              gq = *reinterpret_cast<const uint4*>(gsrc + q * 8);
+              uq = *reinterpret_cast<const uint4*>(gsrc + p.F + q * 8);
+            }
             const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
             float og[8], ou[8];
 #pragma unroll
@@ -289,8 +365,56 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
               ou[2 * i] = d0 * g0 * s0;
               ou[2 * i + 1] = d1 * g1 * s1;
             }
-            *reinterpret_cast<uint4*>(dgdst + q * 8) = pack8(og);
-            *reinterpret_cast<uint4*>(dgdst + p.F + q * 8) = pack8(ou);
+            dgp[half * 4 + q] = pack8(og);
+            dup[half * 4 + q] = pack8(ou);
+            if (row_ok) {
+              *reinterpret_cast<uint4*>(dgdst + q * 8) = dgp[half * 4 + q];
+              *reinterpret_cast<uint4*>(dgdst + p.F + q * 8) = dup[half * 4 + q];
+            }
+          }
+        }
+        if (p.q_codes) {
+          // fused Q-dgu (R9): 1 x 128 blocks of [dg | du] along 2F; this tile's 128 columns are exactly one block of dg and
+          // one of du, shared with the other column-half warp of the lane group.
+          float amg = 0.f, amu = 0.f;
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const uint32_t wg[4] = {dgp[q].x, dgp[q].y, dgp[q].z, dgp[q].w}, wu[4] = {dup[q].x, dup[q].y, dup[q].z, dup[q].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              amg = fmaxf(amg, fmaxf(fabsf(bf16_lo(wg[i])), fabsf(bf16_hi(wg[i]))));
+              amu = fmaxf(amu, fmaxf(fabsf(bf16_lo(wu[i])), fabsf(bf16_hi(wu[i]))));
+            }
+          }
+          float* slot = xch + ((t & 1) * 2 * BM) * 2;                   // [parity][g|u][row][ch]
+          slot[(0 * BM + row_in_tile) * 2 + ch] = amg;
+          slot[(1 * BM + row_in_tile) * 2 + ch] = amu;
+          named_bar_sync(1 + lg, 64);
+          const float sg = fp8_block_scale(fmaxf(slot[(0 * BM + row_in_tile) * 2], slot[(0 * BM + row_in_tile) * 2 + 1]), p.q_mode);
+          const float su = fp8_block_scale(fmaxf(slot[(1 * BM + row_in_tile) * 2], slot[(1 * BM + row_in_tile) * 2 + 1]), p.q_mode);
+          const float isg = 1.0f / sg, isu = 1.0f / su;
+          if (row_ok) {
+            uint8_t* cg = p.q_codes + row * (int64_t)(2 * p.F) + tl.n0 + ch * 64;
+            uint8_t* cu = cg + p.F;
+#pragma unroll
+            for (int q = 0; q < 8; q += 2) {
+              uint32_t eg[4], eu[4];
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const uint4 vg = dgp[q + h], vu = dup[q + h];
+                eg[2 * h] = enc4(bf16_lo(vg.x), bf16_hi(vg.x), bf16_lo(vg.y), bf16_hi(vg.y), sg, isg, p.q_mode);
+                eg[2 * h + 1] = enc4(bf16_lo(vg.z), bf16_hi(vg.z), bf16_lo(vg.w), bf16_hi(vg.w), sg, isg, p.q_mode);
+                eu[2 * h] = enc4(bf16_lo(vu.x), bf16_hi(vu.x), bf16_lo(vu.y), bf16_hi(vu.y), su, isu, p.q_mode);
+                eu[2 * h + 1] = enc4(bf16_lo(vu.z), bf16_hi(vu.z), bf16_lo(vu.w), bf16_hi(vu.w), su, isu, p.q_mode);
+              }
+              *reinterpret_cast<uint4*>(cg + q * 8) = make_uint4(eg[0], eg[1], eg[2], eg[3]);
+              *reinterpret_cast<uint4*>(cu + q * 8) = make_uint4(eu[0], eu[1], eu[2], eu[3]);
+            }
+            if (ch == 0) {
+              float* sc = p.q_scales + row * (int64_t)(2 * p.F / 128);
+              sc[tl.n0 / 128] = sg;
+              sc[(p.F + tl.n0) / 128] = su;
+            }
           }
         }
       }
@@ -350,6 +474,10 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
   p.ldgu = c.ldgu;
   p.p2f = c.p2f;
   p.w = c.w;
+  p.q_codes = c.q_codes;
+  p.q_scales = c.q_scales;
+  p.q_mode = c.q_mode;
+  if (c.q_codes && (!c.q_scales || c.F % 128 != 0)) return MOE_ERR_INVALID_ARG;
   CUtensorMap ta, tb0, tb1;
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
   const int64_t wrows = (int64_t)c.E * c.b_rows;

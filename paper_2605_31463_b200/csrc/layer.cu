@@ -1,6 +1,7 @@
 // moe_layer_fwd / moe_layer_bwd: composition of the hot path (SURVEY.md §3 call stack, §8c R1..R8),
 // plus the public grouped-GEMM entry points.  Single stream, no host synchronisation anywhere:
 // per-expert counts stay on the device.
+#include <stdlib.h>
 #include <string.h>
 
 #include "fp8.cuh"
@@ -148,6 +149,17 @@ struct Fp8Bufs {
   int mode;
 };
 
+// Quantise-in-epilogue vs the stand-alone quantiser passes for Q-a / Q-dgu.  Both give the same bits
+// (tests/test_gpu_fp8.py).  With power-of-two scales the epilogue quantises by an exact multiplication and is the
+// default; with fp32 scales (mode 0) every code needs an IEEE division on the promotion warps' critical path, which costs
+// the two GEMMs more (+0.55 / +0.76 ms on configs[3]) than the two HBM passes it removes (-0.65 ms), so the stand-alone
+// passes stay the default there.  MOE_B200_FP8_FUSED_QUANT=0/1 forces either (debug knob, not part of the ABI).
+bool fused_quant(int scale_mode) {
+  const char* e = getenv("MOE_B200_FP8_FUSED_QUANT");     // read per call: tests flip it inside one process
+  if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
+  return scale_mode == 1;
+}
+
 F8Call f8_base(const FfnGroup& g, int mode) {
   F8Call c;
   memset(&c, 0, sizeof(c));
@@ -163,10 +175,14 @@ int32_t ffn_fwd_fp8(const FfnGroup& g, const Fp8Bufs& q, void* gu, void* a, void
   F8Call c = f8_base(g, F8_FWD_SWIGLU);   // gu = [Q(X) Q(Wg)^T | Q(X) Q(Wu)^T], a = silu(g) * u
   c.A = q.Aq; c.lda = g.H; c.a_scales = q.Aq_s; c.B0 = q.Wgq; c.b0_scales = q.Wgq_s; c.B1 = q.Wuq; c.b1_scales = q.Wuq_s;
   c.b_rows = g.F; c.b_cols = g.H; c.N = g.F; c.out0 = gu; c.ld0 = 2 * g.F; c.out1 = a; c.ld1 = g.F;
+  const bool fused = fused_quant(q.mode);
+  if (fused) { c.q_codes = q.aq; c.q_scales = q.aq_s; c.q_mode = q.mode; }   // Q-a on the bf16 a, in the epilogue
   MOE_CHECK(fp8_gemm(c, s));
   prof_mark(g.st_fwd1, s);
-  MOE_CHECK(fp8_quantize_act(a, g.rows_cap, g.F, q.mode, q.aq, q.aq_s, s));   // Q-a on the bf16 a
-  prof_mark(ST_QUANT, s);
+  if (!fused) {
+    MOE_CHECK(fp8_quantize_act(a, g.rows_cap, g.F, q.mode, q.aq, q.aq_s, s));   // Q-a as a stand-alone pass
+    prof_mark(ST_QUANT, s);
+  }
   c = f8_base(g, F8_FWD);                 // y = Q(a) Q(Wd)^T
   c.A = q.aq; c.lda = g.F; c.a_scales = q.aq_s; c.B0 = q.Wdq; c.b0_scales = q.Wdq_s; c.b_rows = g.H; c.b_cols = g.F;
   c.N = g.H; c.out0 = y; c.ld0 = g.H;
@@ -181,10 +197,14 @@ int32_t ffn_bwd_fp8(const FfnGroup& g, const Fp8Bufs& q, const void* dy, const v
   F8Call c = f8_base(g, F8_DGRAD_SWIGLU);  // dgu = swiglu'(gu) * w_r * (Q(dY)[t_r] Q(Wd)[e])
   c.A = q.dyq; c.lda = g.H; c.a_scales = q.dyq_s; c.B0 = q.Wdq; c.b0_scales = q.Wdq_s; c.b_rows = g.H; c.b_cols = g.F;
   c.N = g.F; c.gu = gu; c.ldgu = 2 * g.F; c.out0 = dgu; c.ld0 = 2 * g.F; c.p2f = q.p2f; c.w = q.w;
+  const bool fused = fused_quant(q.mode);
+  if (fused) { c.q_codes = q.dguq; c.q_scales = q.dguq_s; c.q_mode = q.mode; }   // Q-dgu in the epilogue
   MOE_CHECK(fp8_gemm(c, s));
   prof_mark(g.st_bwd1, s);
-  MOE_CHECK(fp8_quantize_act(dgu, g.rows_cap, 2 * g.F, q.mode, q.dguq, q.dguq_s, s));   // Q-dgu
-  prof_mark(ST_QUANT, s);
+  if (!fused) {
+    MOE_CHECK(fp8_quantize_act(dgu, g.rows_cap, 2 * g.F, q.mode, q.dguq, q.dguq_s, s));   // Q-dgu as a stand-alone pass
+    prof_mark(ST_QUANT, s);
+  }
   c = f8_base(g, F8_DGRAD);                // dXp = Q(dg) Q(Wg)[e] + Q(du) Q(Wu)[e]
   c.A = q.dguq; c.lda = 2 * g.F; c.a_scales = q.dguq_s; c.B0 = q.Wgq; c.b0_scales = q.Wgq_s; c.B1 = q.Wuq;
   c.b1_scales = q.Wuq_s; c.b_rows = g.F; c.b_cols = g.H; c.N = g.H; c.out0 = dXp; c.ld0 = g.H;

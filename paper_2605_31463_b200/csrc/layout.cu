@@ -191,12 +191,14 @@ extern "C" int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size
       {"perm_to_flat", L.p2f, R * 4}, {"flat_to_perm", L.f2p, T * cfg->K * 4}, {"Xp", L.Xp, R * H * es},
       {"gu", L.gu, R * 2 * F * es}, {"a", L.a, R * F * es}, {"y", L.y, R * H * es},
       {"gu_s", L.gu_s, T * 2 * Fs * es}, {"a_s", L.a_s, T * Fs * es}, {"y_s", L.y_s, T * H * es},
-      {"aux_f", L.aux_f, E * 4}, {"aux_P", L.aux_P, E * 4}, {"aux_loss", L.aux_loss, 4}};
+      {"aux_f", L.aux_f, E * 4}, {"aux_P", L.aux_P, E * 4}, {"aux_loss", L.aux_loss, 4},
+      {"aq", L.aq, R * F}, {"aq_s", L.aq_s, R * (F / 128) * 4}};
   for (auto& t : tab)
     if (strcmp(t.n, name) == 0) {
       const size_t nl = strlen(name);
       if (nl > 2 && strcmp(name + nl - 2, "_s") == 0 && !Fs) return MOE_ERR_INVALID_ARG;
       if (strncmp(name, "aux_", 4) == 0 && cfg->aux_coef == 0.f) return MOE_ERR_INVALID_ARG;
+      if (strncmp(name, "aq", 2) == 0 && cfg->dtype != 2) return MOE_ERR_INVALID_ARG;
       *byte_offset = t.off;
       *byte_len = t.len;
       return MOE_OK;
@@ -212,10 +214,12 @@ extern "C" int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_
   const size_t R = (size_t)padded_rows(cfg), T = cfg->T, H = cfg->H, F = cfg->F;
   struct { const char* n; size_t off, len; } tab[] = {
       {"dw", L.dw, T * cfg->K * 4}, {"dz", L.dz, T * cfg->K * 4}, {"dy", L.dy, R * H * es},
-      {"dgu", L.dgu, R * 2 * F * es}, {"dXp", L.dXp, R * H * es}, {"dz_dense", L.dzd, T * (size_t)cfg->E * 4}};
+      {"dgu", L.dgu, R * 2 * F * es}, {"dXp", L.dXp, R * H * es}, {"dz_dense", L.dzd, T * (size_t)cfg->E * 4},
+      {"dguq", L.dguq, R * 2 * F}, {"dguq_s", L.dguq_s, R * (2 * F / 128) * 4}};
   for (auto& t : tab)
     if (strcmp(t.n, name) == 0) {
       if (strcmp(name, "dz_dense") == 0 && !dense_router_bwd(cfg)) return MOE_ERR_INVALID_ARG;
+      if (strncmp(name, "dguq", 4) == 0 && cfg->dtype != 2) return MOE_ERR_INVALID_ARG;
       *byte_offset = t.off;
       *byte_len = t.len;
       return MOE_OK;

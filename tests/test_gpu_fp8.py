@@ -127,6 +127,29 @@ def test_fp8_layer_fwd_bwd_matches_fake_quant_oracle(cfg):
     print(cfg.name, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
 
 
+@pytest.mark.parametrize("fused", ["0", "1"])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_fused_epilogue_quantisers_are_bit_exact(env, mode, fused, monkeypatch):
+    """PAPER.md:116 fused FP8 quantisation: the codes and 1x128 scales that the GEMM-1 epilogue emits for `a` (Q-a) and
+    the dgrad-down epilogue for [dg|du] (Q-dgu) are the SAME BITS the oracle's quantiser gives on the bf16 tensors those
+    kernels wrote (rows of real tokens and padding rows; the shared expert's single-group path included)."""
+    torch, moe, buffers = env
+    monkeypatch.setenv("MOE_B200_FP8_FUSED_QUANT", fused)      # "1": quantise in the epilogues; "0": stand-alone passes
+    cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode)
+    inp = gc.gen_inputs(cfg)
+    lb = gc.run_gpu_layer(cfg, inp)
+    gc.compare_layer(cfg, inp, lb)                              # ... and the layer still matches the fake-quant oracle
+    R = int(buffers.to_numpy(lb.ctx_view("offsets"))[-1])
+    a = buffers.to_numpy(lb.ctx_view("a"))[:R]
+    codes, sc = orc.quantize_1x128(a, mode)
+    assert np.array_equal(buffers.to_numpy(lb.ctx_view("aq"))[:R], codes)
+    assert np.array_equal(buffers.to_numpy(lb.ctx_view("aq_s"))[:R], sc)
+    dgu = buffers.to_numpy(lb.ws_view("dgu"))[:R]
+    codes, sc = orc.quantize_1x128(dgu, mode)
+    assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq"))[:R], codes)
+    assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq_s"))[:R], sc)
+
+
 def test_fp8_weight_cache_matches_oracle(env):
     """FP8 weight cache: quantise the weights once with moe_fp8_quantize_weights, then run a NEW
     micro-batch through moe_layer_fwd with NULL weights (the bf16 weights overwritten with garbage first, so nothing
