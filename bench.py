@@ -223,6 +223,48 @@ def roof(flops, byts, sec, peak_tflops, peak_gbs):
     return bound, max(t_tensor, t_hbm) / sec
 
 
+def time_standalone_movers(moe, lb, cfg, stream, iters=20):
+    """"the standalone moe_permute / moe_unpermute_combine are what the GB/s metric measures even if
+    moe_layer_fwd fuses the gather".  moe_route + moe_permute (histogram, scan, maps, row gather) from the layer's logits,
+    and moe_unpermute_combine on the result, each timed per call with CUDA events on the launching stream; a 512 MB
+    buffer is overwritten between calls (outside the events) so that every call starts with a cold L2."""
+    import torch
+    b = 4 if cfg.dtype == wl.DTYPE_FP32 else 2
+    T, H, E, K, TK = cfg.T, cfg.H, cfg.E, cfg.K, cfg.T * cfg.K
+    R = lb.R
+    z = lb.ctx_view("z").clone()
+    i32 = lambda *sh: torch.empty(*sh, dtype=torch.int32, device="cuda")
+    idx, w = i32(T, K), torch.empty(T, K, dtype=torch.float32, device="cuda")
+    counts, offsets, p2f, f2p = i32(E), i32(E + 1), i32(R), i32(TK)
+    Xp = torch.empty(R, H, dtype=lb.X.dtype, device="cuda")
+    Y = torch.empty_like(lb.X)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t_rp, t_c = [], []
+    for it in range(iters + 3):
+        flush.fill_(it & 0xff)
+        ev[0].record(stream)
+        moe.moe_route(lb.ccfg, z, lb.bias, idx, w, stream)
+        moe.moe_permute(lb.ccfg, lb.X, idx, counts, offsets, p2f, f2p, Xp, lb.ws, stream)
+        ev[1].record(stream)
+        flush.fill_(it & 0xff)
+        ev[2].record(stream)
+        moe.moe_unpermute_combine(lb.ccfg, Xp, w, f2p, None, Y, stream)
+        e3 = torch.cuda.Event(enable_timing=True)
+        e3.record(stream)
+        torch.cuda.synchronize()
+        if it >= 3:
+            t_rp.append(ev[0].elapsed_time(ev[1]))
+            t_c.append(ev[2].elapsed_time(e3))
+    sb = stage_bytes(cfg)
+    med = lambda v: sorted(v)[len(v) // 2]
+    rp_bytes = sb["route"] + sb["maps"] + sb["permute"]
+    return {"route_permute": {"gbs": rp_bytes / (med(t_rp) * 1e-3) / 1e9, "bytes": rp_bytes, "ms": med(t_rp),
+                              "calls": "moe_route + moe_permute, stand-alone, cold L2, median of %d" % iters},
+            "combine": {"gbs": sb["combine"] / (med(t_c) * 1e-3) / 1e9, "bytes": sb["combine"], "ms": med(t_c),
+                        "calls": "moe_unpermute_combine, stand-alone, cold L2, median of %d" % iters}}
+
+
 def run_cuda(args, cfg):
     import torch
     import torch.distributed as dist
@@ -363,6 +405,7 @@ def run_cuda(args, cfg):
            "serial_value": world * fl["total"] * args.steps / (ms_serial * 1e-3) / 1e12,
            "serial_ms_per_step": ms_serial / args.steps}
 
+    standalone = time_standalone_movers(moe, lb, cfg, stream) if rank == 0 else None
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -376,6 +419,10 @@ def run_cuda(args, cfg):
     regime = "burst" if burst else "sustained"
     bf16_peak = peaks["bf16_burst"] if burst else peaks["bf16_sustained"]
     sf, sb = stage_flops(cfg), stage_bytes(cfg)
+    if lb.rows_fused == 1:     # the combine-bwd slot holds a plain gather of dY (+ the dw reduction): permute's bytes
+        sb["combine_bwd"] = sb["permute"]
+    elif lb.rows_fused == 2:   # no permute / combine-bwd pass inside the layer: the slots hold only the dw reduction
+        sb.pop("permute"); sb.pop("combine_bwd")
     traffic, traffic_src = load_traffic(cfg.name)
     gemm_names = ("gemm1_swiglu", "gemm2", "dgrad_down_swiglu", "dgrad_gateup", "wgrad")
 
@@ -432,13 +479,10 @@ def run_cuda(args, cfg):
                         "frac_measured_sustained": tfl / tsec / 1e12 / peaks["bf16_sustained"],
                         "frac_nominal_2250": tfl / tsec / 1e12 / NOMINAL["bf16_tflops"], "stages": gemm_stages,
                         "note": "bf16 denominators; an fp8 config's fprop/dgrad stages have twice that peak"}
-    rp = [stages[n]["ms_per_step"] for n in ("route", "maps", "permute") if n in stages]
-    route_permute = None
-    if len(rp) == 3:
-        byts = sb["route"] + sb["maps"] + sb["permute"]
-        gbs = byts / (sum(rp) * 1e-3) / 1e9
-        route_permute = {"gbs": gbs, "bytes": byts, "ms": sum(rp), "frac_measured": gbs / peaks["hbm_gbs"],
-                         "frac_nominal_8000": gbs / NOMINAL["hbm_gbs"]}
+    route_permute = standalone["route_permute"]
+    for k in ("route_permute", "combine"):
+        standalone[k]["frac_measured"] = standalone[k]["gbs"] / peaks["hbm_gbs"]
+        standalone[k]["frac_nominal_8000"] = standalone[k]["gbs"] / NOMINAL["hbm_gbs"]
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         f, t, desc = oracle_sample(cfg)
@@ -456,7 +500,8 @@ def run_cuda(args, cfg):
             "frac_of_measured_bf16_sustained": value / world / peaks["bf16_sustained"],
             "frac_of_nominal_bf16_2250": value / world / NOMINAL["bf16_tflops"],
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "gemm_all": gemm_all,
-            "route_permute": route_permute, "stages": stages, "cpu_baseline": cpu, "peaks": peaks}
+            "rows_fused": int(lb.rows_fused), "route_permute": route_permute, "combine_standalone": standalone["combine"],
+            "stages": stages, "cpu_baseline": cpu, "peaks": peaks}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

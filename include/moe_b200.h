@@ -88,6 +88,22 @@ int32_t moe_version(void);
  * row_align.  Returns < 0 on an invalid config. */
 int64_t moe_padded_rows(const moe_config_t* cfg);
 
+/* How moe_layer_fwd / bwd / wgrad fold the routing weight and the permutation into the grouped GEMMs for this config
+ * (< 0: invalid config).  PAPER.md:116 ("fused ... token scatter"); BASELINE.json north_star (3) "routing-weight scaling
+ * fused into the epilogues".
+ *  0  nothing fused (fp32, FP8, unaligned groups, zero-computation experts; or MOE_B200_FUSED_ROWS=0): w is applied in the
+ *     combine, the backward starts with a combine-backward pass writing dy = w dY and dw.
+ *  1  (default for bf16 with H, F multiples of 64 and row_align a multiple of 128): the routing weight is applied in the
+ *     GEMM-1 epilogue (ctx "a" holds w_r a_r, ctx "y" holds w_r y_r, the combine is a plain sum over the K rows) and in the
+ *     dgrad-down epilogue, which also produces dw[t,j] = <da_r, a_r> (= <dY_t, y_r>, R8).  The combine-backward pass is
+ *     replaced by a plain row gather of dY: ws "dy" holds the UNWEIGHTED rows of dY, y is not read by the backward.
+ *  2  (MOE_B200_FUSED_ROWS=2) as 1, and GEMM-1 gathers the rows of X, dgrad-down the rows of dY, inside the kernel (TMA
+ *     tile::gather4 through perm_to_flat), each writing the row-grouped copy ("Xp", "dy") that the weight gradients contract
+ *     over as a by-product of its staged tiles: no row-mover pass at all.
+ * The layer's results (Y, dX, dW*, dWr, topk_*) mean the same in all three.  The stand-alone moe_permute /
+ * moe_unpermute_combine are not affected. */
+int32_t moe_layer_rows_fused(const moe_config_t* cfg);
+
 /* Bytes of scratch (`ws`, contents undefined between calls) and of saved-for-backward context
  * (`ctx`, written by moe_layer_fwd, read by moe_layer_bwd) for this config.  Both 256-byte multiples. */
 int32_t moe_workspace_bytes(const moe_config_t* cfg, size_t* ws_bytes, size_t* ctx_bytes);

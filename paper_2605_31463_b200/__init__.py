@@ -56,6 +56,7 @@ _SIGNATURES = {
     "moe_version": (_I32, []),
     "moe_launch_count": (_I64, []),
     "moe_padded_rows": (_I64, [_CFG]),
+    "moe_layer_rows_fused": (_I32, [_CFG]),
     "moe_workspace_bytes": (_I32, [_CFG, _SZP, _SZP]),
     "moe_route": (_I32, [_CFG, _P, _P, _P, _P, _P]),
     "moe_route_threshold": (_I32, [_CFG, _P, _P, _P, _P, _P]),
@@ -154,6 +155,13 @@ def moe_padded_rows(cfg) -> int:
     r = lib().moe_padded_rows(C.byref(make_config(cfg)))
     if r < 0:
         raise MoEError(MOE_ERR_INVALID_ARG, "moe_padded_rows")
+    return r
+
+
+def moe_layer_rows_fused(cfg) -> int:
+    r = lib().moe_layer_rows_fused(C.byref(make_config(cfg)))
+    if r < 0:
+        raise MoEError(r, "moe_layer_rows_fused")
     return r
 
 

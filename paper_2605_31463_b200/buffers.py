@@ -5,7 +5,7 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from . import (make_config, make_extras, moe_ctx_field, moe_layer_bwd, moe_layer_bwd_ex, moe_layer_fwd, moe_layer_fwd_ex,
+from . import (make_config, make_extras, moe_ctx_field, moe_layer_rows_fused, moe_layer_bwd, moe_layer_bwd_ex, moe_layer_fwd, moe_layer_fwd_ex,
                moe_layer_step_host,
                moe_layer_step_host_pipelined, moe_padded_rows, moe_pipeline_create, moe_pipeline_destroy,
                moe_workspace_bytes, moe_ws_field)
@@ -38,6 +38,7 @@ class LayerBuffers:
         dt = act_dtype(cfg)
         T, H, E, K, F, Fs = cfg.T, cfg.H, cfg.E, cfg.K, cfg.F, cfg.F_shared
         self.R = moe_padded_rows(cfg)
+        self.rows_fused = moe_layer_rows_fused(cfg)     # >= 1: ctx "a" / "y" carry the routing weight, ws "dy" is unweighted
         ws_b, ctx_b = moe_workspace_bytes(cfg)
         e = lambda *shape, dtype=dt: torch.empty(*shape, dtype=dtype, device=device)
         self.ws = e(ws_b, dtype=torch.uint8)

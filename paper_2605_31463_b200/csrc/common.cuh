@@ -79,6 +79,17 @@ inline bool dense_router_bwd(const moe_config_t* c) {
   return c->aux_coef != 0.f || n_zc(c) > 0 || (c->score_fn == 0 && !c->renorm && c->route_mode == 0);
 }
 
+// Routing weights FUSED into the grouped GEMMs' epilogues (north_star (3)), for bf16 tensor-core layers:
+//  1 (default): GEMM-1 writes a = w silu(g) u, so y = w y and the combine is a plain sum; the backward replaces the
+//     combine-backward pass (reads y and dY, writes dy = w dY) by a plain row gather of dY (ws "dy" = UNWEIGHTED rows),
+//     dgrad-down applies w in its epilogue and produces dw[t,j] = <da_r, a_r> there, so y is never read again.
+//  2: as 1, and GEMM-1 / dgrad-down gather their A rows from the token-major X / dY themselves (TMA tile::gather4 through
+//     perm_to_flat, gather-warp kernel variants), writing Xp / dy as a by-product of the staged tiles: no row-mover pass at
+//     all.  Measured slower than 1 (the by-product stores cost the GEMMs more than the passes they
+//     replace), kept selectable with MOE_B200_FUSED_ROWS=2.
+//  0 (MOE_B200_FUSED_ROWS=0, and every other dtype / layout): w in the combine, dy = w dY from combine-backward.
+int rows_fused(const moe_config_t* c);   // layout.cu
+
 // ---- byte layout of ctx / ws ---------------------------------------------------------------
 struct CtxLayout {
   size_t z, idx, w, counts, offsets, p2f, f2p, mtile, Xp, gu, a, y, gu_s, a_s, y_s;
@@ -90,6 +101,7 @@ struct CtxLayout {
 };
 struct WsLayout {
   size_t hist, tmp, dw, dz, dzp, dwr_part, dy, dgu, dXp, dgu_s, dXs, dYq, dYq_s, dyq, dyq_s, dguq, dguq_s, dgusq, dgusq_s;
+  size_t dwpart;                    // fused rows: fp32 [2 ceil(F/256), R] partial <da, a> sums of the dgrad-down epilogue
   size_t dzd, dzb, dXr, aux_part;  // dense router backward: dz fp32 [T,E], its bf16 copy [T,Ep], dz Wr [T,H]; aux partials
   size_t total;
 };
@@ -107,6 +119,8 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
                     const int32_t* offsets, void* Xp, cudaStream_t s);
 int32_t combine(const moe_config_t* c, const void* y, const float* w, const int32_t* f2p, const void* add0,
                 const void* add1, const float* dz, const int32_t* idx, const void* Wr, void* Y, cudaStream_t s);
+// dw[p] = sum_k part[k, f2p[p]] (fixed order; an empty slot gets 0): the routing-weight gradient from the dgrad-down epilogue
+int32_t dw_reduce(const moe_config_t* c, const float* part, int nparts, const int32_t* f2p, float* dw, cudaStream_t s);
 int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const float* w, const int32_t* f2p,
                     const int32_t* p2f, const int32_t* offsets, void* dy, float* dw, cudaStream_t s);
 // route.cu: moe_route with an optional second copy of the outputs

@@ -121,6 +121,13 @@ struct TcParams {
   int64_t ld1;
   const __nv_bfloat16* gu;
   int64_t ldgu;
+  // fused permutation ("fused token scatter"; north_star: routing weights in the epilogues)
+  const int32_t* gidx;     // perm_to_flat [rows]: flat position t*K+j of a permuted row, -1 = padding row; nullptr = off
+  int gat;                 // 1: the K-major A operand is GATHERED through gidx from token-major rows (gather-warp kernels)
+  int copy_out;            // gathered A tiles are also stored to the row-grouped copy behind tmC (Xp / dy), each k-block once
+  int gshift, gK;          // flat position -> token row: p >> gshift (K a power of two) or p / gK (gshift < 0)
+  const float* roww;       // routing weights by flat position [T*K] (nullptr = 1): FWD_SWIGLU a *= w; DGRAD_SWIGLU dgu *= w
+  float* dwpart;           // DGRAD_SWIGLU: [2 * n_tiles, rows_valid] partial sums of <da, silu(g) u> per row (nullptr = off)
 };
 
 struct Tile {
@@ -167,6 +174,21 @@ __device__ __forceinline__ int64_t total_tiles(const TcParams& p) {
   else if (p.mtile) mt = PAIR ? 0 : p.mtile[0];
   else mt = (p.rows_valid + (PAIR ? 2 * BM : BM) - 1) / (PAIR ? 2 * BM : BM);
   return mt * p.n_tiles;
+}
+
+// Token rows of the four permuted rows r .. r+3 (r a multiple of 4): the TMA gather coordinates of one lane.  A padding
+// row keeps a negative coordinate, which is out of bounds and therefore reads as zeros.
+__device__ __forceinline__ void gather_rows4(const TcParams& p, int64_t r, int (&t)[4]) {
+  const int4 v = __ldg(reinterpret_cast<const int4*>(p.gidx + r));
+  const int f[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) t[i] = f[i] < 0 ? -1 : (p.gshift >= 0 ? f[i] >> p.gshift : f[i] / p.gK);
+}
+// routing weight of permuted row r (0 for a padding row); 1 when the launch carries no weights
+__device__ __forceinline__ float row_weight(const TcParams& p, int64_t r) {
+  if (!p.roww) return 1.0f;
+  const int f = r < p.rows_valid ? __ldg(p.gidx + r) : -1;
+  return f >= 0 ? __ldg(p.roww + f) : 0.0f;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -266,7 +288,7 @@ __device__ __forceinline__ void pack32_to_box(uint32_t rowaddr, int sw, const ui
 
 __device__ __forceinline__ void fwd_swiglu_tile_tma(const TcParams& p, const Tile& tl, uint32_t tacc, int row_in_tile,
                                                     uint32_t obuf, const CUtensorMap* tmGU, const CUtensorMap* tmAo,
-                                                    bool issuer, int ch) {
+                                                    bool issuer, int ch, float wrow) {
   const uint32_t rowaddr = obuf + row_in_tile * 64;
   const int sw = (row_in_tile >> 1) & 3;
 #pragma unroll 1
@@ -290,7 +312,7 @@ __device__ __forceinline__ void fwd_swiglu_tile_tma(const TcParams& p, const Til
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
       const float gv = __uint_as_float(g[i]);
-      g[i] = __float_as_uint(gv * fast_sigmoid(gv) * __uint_as_float(u[i]));
+      g[i] = __float_as_uint(gv * fast_sigmoid(gv) * __uint_as_float(u[i]) * wrow);   // wrow = 1 unless w is folded into a
     }
     if (issuer) bulk_wait_read0();
     named_bar_sync(1 + ch, 128);
@@ -390,7 +412,7 @@ __device__ __forceinline__ void dgrad_swiglu_chunk(const TcParams& p, const Tile
 // leave by TMA store.  No per-thread global loads or stores at all.
 __device__ __forceinline__ void dgrad_swiglu_chunk_tma(const TcParams& p, const Tile& tl, int c, uint32_t tacc, uint32_t obuf,
                                                        int row_in_tile, uint32_t gbar, uint32_t& gphase,
-                                                       const CUtensorMap* tmO, bool issuer, int ch) {
+                                                       const CUtensorMap* tmO, bool issuer, int ch, float wrow, float& dwacc) {
   uint32_t d[32];
   tmem_ld32(tacc + c * 32, d);
   mbar_wait(gbar, gphase);           // g, u of this chunk have landed
@@ -409,8 +431,11 @@ __device__ __forceinline__ void dgrad_swiglu_chunk_tma(const TcParams& p, const 
       const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
       const float d0 = __uint_as_float(d[q * 8 + 2 * i]), d1 = __uint_as_float(d[q * 8 + 2 * i + 1]);
       const float s0 = fast_sigmoid(g0), s1 = fast_sigmoid(g1);
-      og[i] = pack_bf16(d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
-      ou[i] = pack_bf16(d0 * g0 * s0, d1 * g1 * s1);
+      const float a0 = g0 * s0, a1 = g1 * s1;                          // silu(g)
+      dwacc = fmaf(d0, a0 * u0, fmaf(d1, a1 * u1, dwacc));             // <da, a>: the routing weight's gradient (R8)
+      const float e0 = wrow * d0, e1 = wrow * d1;                      // da of the weighted row (wrow = 1: w not folded)
+      og[i] = pack_bf16(e0 * u0 * s0 * (1.0f + g0 * (1.0f - s0)), e1 * u1 * s1 * (1.0f + g1 * (1.0f - s1)));
+      ou[i] = pack_bf16(e0 * a0, e1 * a1);
     }
     st_shared_v4(ga, og[0], og[1], og[2], og[3]);
     st_shared_v4(ua, ou[0], ou[1], ou[2], ou[3]);
@@ -531,11 +556,11 @@ __device__ __forceinline__ void wgrad_accum_tile(const TcParams& p, const Tile& 
 //   issued by the leader (rank 0): each CTA stages its own 128 rows of A and one half of B; TMA bytes of both CTAs are
 //   signalled on the leader's full barrier; tcgen05.commit multicasts "stage free" / "accumulator ready" to both CTAs;
 //   each CTA's epilogue warps drain their own 128 TMEM lanes and release the accumulator on the leader's barrier.
-template <int MODE, bool PAIR>
-__global__ void __launch_bounds__(NTHREADS, 1)
+template <int MODE, bool PAIR, int GW>
+__global__ void __launch_bounds__(NTHREADS + (GW > 0 ? 32 * (GW + 1) : 0), 1)
 tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
                const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmO,
-               const __grid_constant__ CUtensorMap tmO2, const TcParams p) {
+               const __grid_constant__ CUtensorMap tmO2, const __grid_constant__ CUtensorMap tmC, const TcParams p) {
   constexpr bool A_MN = (MODE == TC_WGRAD);
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
   constexpr int STAGES = Ring<PAIR>::STAGES, STAGE_BYTES = Ring<PAIR>::STAGE_BYTES, B_CTA = Ring<PAIR>::B_CTA;
@@ -561,7 +586,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     tma_prefetch_desc(&tmO2);
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full0 + 8 * s, 1);
-      mbar_init(empty0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, (GW > 0 && p.copy_out) ? 2 : 1);   // MMA commit (+ the copy-out warp's store has read the stage)
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull0 + 8 * a, 1);
@@ -585,13 +610,14 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const int64_t total = total_tiles<MODE, PAIR>(p);
 
   if (warp == 0) {
-    // ===================== TMA producer (one thread per CTA) =====================
+    // ===================== TMA producer (one thread per CTA): every operand that is tiled in HBM =====================
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
       // the next tile's schedule entry (two dependent global loads) is fetched while this tile's k-loop runs
       Tile tl, nx;
       bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+      const bool a_tiled = !(GW > 0 && p.gat == 1);   // else: the gather warps' job
       for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
         okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
         const int bn0 = tl.n0 + (PAIR ? rank * (BN / 2) : 0);   // first of the B columns this CTA stages
@@ -609,12 +635,14 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             if (PAIR) tma_load_2d_pair(dst, m, fb, c0, c1);
             else tma_load_2d(dst, m, fb, c0, c1);
           };
-          if (!A_MN) {
-            load(sa, &tmA, kb * BK, tl.m0);                                        // box 64 x 128
-          } else {
-            const int kr = tl.row0 + kb * BK;
+          if (a_tiled) {
+            if (!A_MN) {
+              load(sa, &tmA, kb * BK, tl.m0);                                        // box 64 x 128
+            } else {
+              const int kr = tl.row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BM / 64; ++i) load(sa + i * MN_BOX_BYTES, &tmA, p.a_col0 + tl.m0 + 64 * i, kr);
+              for (int i = 0; i < BM / 64; ++i) load(sa + i * MN_BOX_BYTES, &tmA, p.a_col0 + tl.m0 + 64 * i, kr);
+            }
           }
           if (MODE == TC_FWD || MODE == TC_FWD_F32) {
             load(sb, &tmB0, kb * BK, tl.e * p.b_rows + bn0);                       // box 64 x 256 (pair: 64 x 128)
@@ -675,7 +703,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (++as == 2) { as = 0; aphase ^= 1; }
       }
     }
-  } else {
+  } else if (warp < 2 + EPI_WARPS) {
     // ===================== epilogue warps 2..9 =====================
     const int lg = warp & 3;                 // TMEM lane group this warp may access
     const int ch = (warp - 2) >> 2;          // which half of the column chunks this warp drains
@@ -702,20 +730,24 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int64_t row = (int64_t)tl.m0 + row_in_tile;
         const bool row_ok = row < p.rows_valid;
         constexpr int NC = BN / 64;              // chunks per warp: this warp drains columns [ch * 128, ch * 128 + 128)
-        if (p.tma_out) {
+        if (GW > 0 || p.tma_out) {
           const bool issuer = (threadIdx.x & 127) == 64;
           const uint32_t obuf = obuf0 + ch * GROUP_OBUF, gbar = gbar0 + 8 * ch;
           const int nvalid = min(NC, (p.F - tl.n0 - ch * (BN / 2) + 31) / 32);      // chunks of this group inside F
           if (issuer && nvalid > 0) gu_tma_fetch(p, tl, ch * NC, obuf, gbar, &tmB1);   // overlaps the rest of the main loop
           __syncwarp();
+          const float wrow = row_weight(p, row);
+          float dwacc = 0.f;
           mbar_wait(tfull0 + 8 * as, aphase);
           tc_fence_after();
           for (int i = 0; i < nvalid; ++i) {
-            dgrad_swiglu_chunk_tma(p, tl, ch * NC + i, tacc, obuf, row_in_tile, gbar, gphase, &tmO, issuer, ch);
+            dgrad_swiglu_chunk_tma(p, tl, ch * NC + i, tacc, obuf, row_in_tile, gbar, gphase, &tmO, issuer, ch, wrow, dwacc);
             if (issuer && i + 1 < nvalid) gu_tma_fetch(p, tl, ch * NC + i + 1, obuf, gbar, &tmB1);
             __syncwarp();
           }
           release_acc(as);
+          // this warp group's share of <da, a> over its 128 columns: part (2 n-tile + ch), summed later in fixed order
+          if (p.dwpart && row_ok) p.dwpart[(int64_t)(2 * (tl.n0 / BN) + ch) * p.rows_valid + row] = dwacc;
           if (++as == 2) { as = 0; aphase ^= 1; }
           continue;
         }
@@ -745,10 +777,11 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         if (have && ++as == 2) { as = 0; aphase ^= 1; }
         continue;
-      } else if (MODE == TC_FWD_SWIGLU && p.tma_out) {
+      } else if (MODE == TC_FWD_SWIGLU && (GW > 0 || p.tma_out)) {
+        const float wrow = row_weight(p, (int64_t)tl.m0 + row_in_tile);
         mbar_wait(tfull0 + 8 * as, aphase);
         tc_fence_after();
-        fwd_swiglu_tile_tma(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, &tmO2, (threadIdx.x & 127) == 64, ch);
+        fwd_swiglu_tile_tma(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, &tmO2, (threadIdx.x & 127) == 64, ch, wrow);
       } else {
         if (have) {
           mbar_wait(tfull0 + 8 * as, aphase);
@@ -764,6 +797,75 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if ((MODE == TC_WGRAD || MODE == TC_FWD || MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_FWD_SWIGLU) &&
         (threadIdx.x & 127) == 64)
       bulk_wait0();   // all TMA stores complete before the CTA retires
+  } else if (GW > 0 && !A_MN && warp < 2 + EPI_WARPS + GW) {
+    // ===================== gather warps (GW > 0): the A operand, rows addressed through the permutation map =====================
+    // A's 16 KB per k-block (128 permuted rows x 64 columns) is 32 units of one tile::gather4 = four token rows x 128 bytes;
+    // the 128-byte swizzle follows the shared-memory address, so the units build the same tile a tiled load would.  A warp
+    // issues one gather4 per ~66 cycles whatever its lane count and the TMA unit accepts one per ~14 cycles (measured), so
+    // the units are dealt round-robin to GW warps (unit = warp + GW * lane).  Padding rows carry a negative (out-of-bounds)
+    // coordinate and read as zeros.
+    const int gw = warp - (2 + EPI_WARPS);
+    const int u0 = gw + lane * GW;
+    if (u0 < 32) {
+      int stage = 0;
+      uint32_t phase = 0;
+      Tile tl, nx;
+      bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+      for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
+        okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
+        int gr[4] = {-1, -1, -1, -1};
+        if (tl.nkb > 0) gather_rows4(p, tl.m0 + 4 * u0, gr);
+        for (int kb = 0; kb < tl.nkb; ++kb) {
+          mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const uint32_t sa = base + stage * STAGE_BYTES;
+          if (PAIR) tma_gather4_pair(sa + u0 * 512, &tmA, mapa_shared(full0 + 8 * stage, 0), kb * BK, gr[0], gr[1], gr[2], gr[3]);
+          else tma_gather4(sa + u0 * 512, &tmA, full0 + 8 * stage, kb * BK, gr[0], gr[1], gr[2], gr[3]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (GW > 0 && !A_MN && !PAIR && warp == 2 + EPI_WARPS + GW) {
+    // ===================== copy-out warp (GW > 0): the permuted copy as a by-product =====================
+    // The gathered A tile of a k-block sits in shared memory in exactly the layout of a tiled TMA box, so it is also stored to
+    // the row-grouped copy (Xp from GEMM-1, the gathered dY from dgrad-down) that the weight gradients contract over -- no
+    // separate permute pass, no second read of X / dY.  The n_tiles CTAs that work on one M-tile share the job: n-tile j
+    // stores the k-blocks with kb % n_tiles == j (each block exactly once, the store traffic spread evenly over all tiles).
+    // A stage is released to the producer once the MMAs (tcgen05.commit) AND its store have read it; two stores in flight.
+    if (lane == 0 && p.copy_out) {
+      int stage = 0, pending = -1;
+      uint32_t phase = 0;
+      Tile tl, nx;
+      bool ok = decode_tile<MODE, PAIR>(p, unit, total, rank, tl), okn = false;
+      for (int64_t t = unit; ok; t += nunits, tl = nx, ok = okn) {
+        okn = decode_tile<MODE, PAIR>(p, t + nunits, total, rank, nx);
+        const int nt = tl.n0 / (MODE == TC_FWD_SWIGLU ? BN / 2 : BN);    // this tile's n-tile index
+        for (int kb = 0; kb < tl.nkb; ++kb) {
+          mbar_wait(full0 + 8 * stage, phase);
+          if (kb % p.n_tiles == nt) {
+            tma_store_2d(&tmC, base + stage * STAGE_BYTES, kb * BK, tl.m0);
+            bulk_commit();
+            if (pending >= 0) {
+              bulk_wait_read1();                       // the store before this one has read its stage
+              mbar_arrive(empty0 + 8 * pending);
+            }
+            pending = stage;
+          } else {
+            if (pending >= 0) {
+              bulk_wait_read0();
+              mbar_arrive(empty0 + 8 * pending);
+              pending = -1;
+            }
+            mbar_arrive(empty0 + 8 * stage);
+          }
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+      if (pending >= 0) {
+        bulk_wait_read0();
+        mbar_arrive(empty0 + 8 * pending);
+      }
+      bulk_wait0();                                    // all stores complete before the CTA retires
+    }
   }
   tc_fence_before();
   __syncwarp();
@@ -784,30 +886,33 @@ bool make_map(CUtensorMap* m, const void* ptr, int64_t inner, int64_t outer, int
   return tc_make_map(m, 2, ptr, inner, outer, ld, BK, box_outer);
 }
 
-bool g_attr_set[MAX_DEVICES][6][2];   // per device: cudaFuncAttributeMaxDynamicSharedMemorySize raised for tc_gemm_kernel<MODE, PAIR>
+constexpr int GATHER_WARPS = 5;       // + 1 copy-out warp: 512 threads, 128 registers each
+bool g_attr_set[MAX_DEVICES][6][2][2];   // per device: MaxDynamicSharedMemorySize raised for tc_gemm_kernel<MODE, PAIR, GW>
 
 // max_units = upper bound on tiles (PAIR: pair-tiles).  PAIR launches clusters of two CTAs (one TPC each).
-template <int MODE, bool PAIR>
-int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
-               int64_t max_units, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
+template <int MODE, bool PAIR, int GW>
+int32_t launch_impl(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
+                    int64_t max_units, cudaStream_t s, const CUtensorMap* o2, const CUtensorMap* cp) {
   const int dev = current_device();
   if (dev < 0) return MOE_ERR_CUDA;
-  if (!g_attr_set[dev][MODE][PAIR]) {
-    MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    g_attr_set[dev][MODE][PAIR] = true;
+  if (!g_attr_set[dev][MODE][PAIR][GW > 0]) {
+    MOE_CUDA(cudaFuncSetAttribute(tc_gemm_kernel<MODE, PAIR, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    g_attr_set[dev][MODE][PAIR][GW > 0] = true;
   }
   const int sms = device_sm_count();
   if (sms <= 0) return MOE_ERR_CUDA;
+  constexpr int NT = NTHREADS + (GW > 0 ? 32 * (GW + 1) : 0);
+  const CUtensorMap& cc = cp ? *cp : a;
   if (!PAIR) {
     const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_units));
-    MOE_LAUNCH((tc_gemm_kernel<MODE, false>), grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, p);
+    MOE_LAUNCH((tc_gemm_kernel<MODE, false, GW>), grid, NT, SMEM_BYTES, s, a, b0, b1, o, o2 ? *o2 : o, cc, p);
     return MOE_OK;
   }
   const unsigned pairs = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms / 2, max_units));
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3(2 * pairs);
-  cfg.blockDim = dim3(NTHREADS);
+  cfg.blockDim = dim3(NT);
   cfg.dynamicSmemBytes = SMEM_BYTES;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
@@ -819,11 +924,24 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
   cfg.numAttrs = 1;
   const CUtensorMap& oo2 = o2 ? *o2 : o;
   ++g_launches;
-  if (cudaLaunchKernelEx(&cfg, tc_gemm_kernel<MODE, true>, a, b0, b1, o, oo2, p) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, tc_gemm_kernel<MODE, true, GW>, a, b0, b1, o, oo2, cc, p) != cudaSuccess) {
     cudaGetLastError();
     return MOE_ERR_CUDA;
   }
   return MOE_OK;
+}
+
+// A launch with a gathered A operand (p.gat) runs the 1-CTA variant with GATHER_WARPS gather warps + one copy-out warp;
+// only the two ragged GEMMs the fused layer feeds from token-major rows (GEMM-1, dgrad-down) have one.
+template <int MODE, bool PAIR>
+int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const CUtensorMap& o, const TcParams& p,
+               int64_t max_units, cudaStream_t s, const CUtensorMap* o2 = nullptr, const CUtensorMap* cp = nullptr) {
+  constexpr bool CAN_GATHER = (MODE == TC_FWD_SWIGLU || MODE == TC_DGRAD_SWIGLU) && !PAIR;
+  if (p.gat != 0) {
+    if constexpr (CAN_GATHER) return launch_impl<MODE, PAIR, GATHER_WARPS>(a, b0, b1, o, p, max_units, s, o2, cp);
+    else return MOE_ERR_UNSUPPORTED;
+  }
+  return launch_impl<MODE, PAIR, 0>(a, b0, b1, o, p, max_units, s, o2, nullptr);
 }
 
 // Which launches use the CTA-pair kernel.  Default 1: the weight gradients (no ragged dimension: every 256 x 256 tile
@@ -843,12 +961,13 @@ int pair_mode() {
 // 1-CTA kernel over the unpaired M-tiles.  With `pl == nullptr` (no pair table) the 1-CTA kernel runs all tiles.
 template <int MODE>
 int32_t launch_both(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b0_pair, const CUtensorMap& b1,
-                    const CUtensorMap& o, TcParams p, const TcCall& c, cudaStream_t s, const CUtensorMap* o2 = nullptr) {
+                    const CUtensorMap& o, TcParams p, const TcCall& c, cudaStream_t s, const CUtensorMap* o2 = nullptr,
+                    const CUtensorMap* cp = nullptr) {
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
   const bool grouped = c.mtile != nullptr;
-  if (pair_mode() == 0 || (grouped && (pair_mode() < 2 || !c.plist || !c.olist))) {
+  if (pair_mode() == 0 || p.gat || (grouped && (pair_mode() < 2 || !c.plist || !c.olist))) {   // gathered A: 1-CTA kernel
     p.tlist = nullptr;
-    return launch<MODE, false>(a, b0, b1, o, p, max_mtiles * p.n_tiles, s, o2);
+    return launch<MODE, false>(a, b0, b1, o, p, max_mtiles * p.n_tiles, s, o2, cp);
   }
   if (!grouped) {       // one group of rows_cap rows from row 0: pairs of consecutive M-tiles cover it
     p.tlist = nullptr;
@@ -899,7 +1018,22 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
   p.M = c.M;
   p.b_rows = c.b_rows;
   p.a_col0 = c.a_col0;
-  CUtensorMap ta, tb0, tb0p, tb1, to;
+  p.gidx = c.gidx;
+  p.gat = c.gat;
+  p.gK = c.gK > 0 ? c.gK : 1;
+  p.gshift = -1;
+  for (int sh = 0; sh < 31; ++sh)
+    if ((1 << sh) == p.gK) p.gshift = sh;
+  p.roww = c.roww;
+  p.dwpart = c.dwpart;
+  p.copy_out = (c.gat && c.copy_out) ? 1 : 0;
+  if (c.gat < 0 || c.gat > 1 || (c.gat && c.mode != TC_FWD_SWIGLU && c.mode != TC_DGRAD_SWIGLU)) return MOE_ERR_INVALID_ARG;
+  if ((c.gat || c.roww) && (!c.gidx || !c.mtile)) return MOE_ERR_INVALID_ARG;
+  if (c.gat && (c.g_rows <= 0 || (reinterpret_cast<uintptr_t>(c.gidx) & 15))) return MOE_ERR_INVALID_ARG;
+  if (c.copy_out && !c.gat) return MOE_ERR_INVALID_ARG;
+  const int64_t a_rows = c.gat == 1 ? c.g_rows : c.rows_cap;     // rows of the tensor behind the A map
+  const int a_box = c.gat == 1 ? 1 : BM;                          // gathered: box = one row of 64 columns (x4 per gather4)
+  CUtensorMap ta, tb0, tb0p, tb1, to, tc;
   if (c.mode == TC_FWD_F32 ? ((c.N & 3) || (c.ld0 & 3)) : ((c.N & 7) || (c.ld0 & 7))) return MOE_ERR_UNSUPPORTED;
   switch (c.mode) {
     case TC_FWD_F32:
@@ -907,7 +1041,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (c.Kd % BK) return MOE_ERR_UNSUPPORTED;
       p.nkb = c.Kd / BK;
       p.n_tiles = (int)ceil_div(c.N, BN);
-      if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&ta, c.A, c.Kd, a_rows, c.lda, a_box)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0p, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;   // a pair CTA's half
       if (c.mode == TC_FWD_F32) return launch_both<TC_FWD_F32>(ta, tb0, tb0p, tb0, ta, p, c, s);
@@ -918,7 +1052,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (c.Kd % BK || (c.F & 7) || (c.ld1 & 7)) return MOE_ERR_UNSUPPORTED;
       p.nkb = c.Kd / BK;
       p.n_tiles = (int)ceil_div(c.F, BN / 2);
-      if (!make_map(&ta, c.A, c.Kd, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&ta, c.A, c.Kd, a_rows, c.lda, a_box)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, c.B1, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, BN / 2)) return MOE_ERR_UNSUPPORTED;
       p.tma_out = (c.F % 32 == 0) ? 1 : 0;   // g / u boxes of 32 columns must not straddle the [g|u] boundary
@@ -926,8 +1060,10 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (p.tma_out && (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM) ||    // gu [rows, 2F]
                         !tc_make_map3(&to2, 2, c.out1, c.F, c.rows_cap, 1, c.ld1, 32, BM)))                  // a [rows, F]
         p.tma_out = 0;
+      if (!p.tma_out && (c.roww || c.gat)) return MOE_ERR_UNSUPPORTED;   // weighted epilogue / gather variant: TMA-store path only
+      if (p.copy_out && !make_map(&tc, c.copy_out, c.Kd, c.rows_cap, c.ld_copy, BM)) return MOE_ERR_UNSUPPORTED;   // Xp [rows, H]
       if (!p.tma_out) return launch_both<TC_FWD_SWIGLU>(ta, tb0, tb0, tb1, ta, p, c, s);
-      return launch_both<TC_FWD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s, &to2);
+      return launch_both<TC_FWD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s, &to2, p.copy_out ? &tc : nullptr);
     }
     case TC_DGRAD:
     case TC_DGRAD_SWIGLU: {
@@ -937,7 +1073,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       p.kb_split = c.b_rows / BK;
       p.nkb = split ? 2 * p.kb_split : p.kb_split;
       p.n_tiles = (int)ceil_div(c.N, BN);
-      if (!make_map(&ta, c.A, (int64_t)p.nkb * BK, c.rows_cap, c.lda, BM)) return MOE_ERR_UNSUPPORTED;
+      if (!make_map(&ta, c.A, (int64_t)p.nkb * BK, a_rows, c.lda, a_box)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb0, c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (!make_map(&tb1, split ? c.B1 : c.B0, c.b_cols, (int64_t)c.E * c.b_rows, c.b_cols, 64)) return MOE_ERR_UNSUPPORTED;
       if (c.mode == TC_DGRAD) {
@@ -949,8 +1085,10 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       if (p.tma_out && !split &&                                                          // saved [g|u] rows, same boxes
           !tc_make_map3(&tb1, 2, c.gu, 2 * (int64_t)c.F, c.rows_cap, 1, c.ldgu, 32, BM))
         p.tma_out = 0;
+      if (!p.tma_out && (c.roww || c.dwpart || c.gat)) return MOE_ERR_UNSUPPORTED;
+      if (p.copy_out && !make_map(&tc, c.copy_out, (int64_t)p.nkb * BK, c.rows_cap, c.ld_copy, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map3(&to, 2, c.out0, 2 * (int64_t)c.F, c.rows_cap, 1, c.ld0, 32, BM)) return MOE_ERR_UNSUPPORTED;   // dgu [rows, 2F]
-      return launch_both<TC_DGRAD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s);
+      return launch_both<TC_DGRAD_SWIGLU>(ta, tb0, tb0, tb1, to, p, c, s, nullptr, p.copy_out ? &tc : nullptr);
     }
     case TC_WGRAD: {
       // every (expert, 256 x 256 output tile) goes to a CTA pair: no ragged dimension, the contraction runs over the

@@ -40,6 +40,17 @@ struct TcCall {
   const void* gu; int ldgu;  // DGRAD_SWIGLU: saved [g|u]
   int F;                     // SwiGLU width
   int acc_f32;               // WGRAD: out0 is fp32 [E,M,N] and the tile is ADDED to it (ld0 in fp32 elements)
+  // --- fused permutation (PAPER.md:116 fused token scatter; optional; FWD_SWIGLU and DGRAD_SWIGLU of grouped launches) ---
+  const int32_t* gidx;       // perm_to_flat [rows_cap] (device): flat position t*K+j of each row, -1 = padding row
+  int gat;                   // 1: A is the TOKEN-major tensor [g_rows, lda]; its rows are gathered by TMA (tile::gather4)
+                             // through gidx inside the kernel; 0: A is row-grouped already
+  int gK;                    // top-k: token row = flat position / gK
+  int64_t g_rows;            // rows of the token-major tensor (T)
+  void* copy_out; int ld_copy;   // gat: the gathered rows are also written here, row-grouped [rows_cap, ld_copy] (padding rows
+                             // as zeros): Xp from GEMM-1, the gathered dY from dgrad-down, for the weight gradients.  NULL = off
+  const float* roww;         // routing weights by flat position [T*K] (needs gidx): FWD_SWIGLU writes a = w silu(g) u,
+                             // DGRAD_SWIGLU writes dgu = w swiglu'(gu) da
+  float* dwpart;             // DGRAD_SWIGLU: fp32 [2 * ceil(F / 256), rows_cap] partial sums of <da, silu(g) u> (dw, R8)
 };
 
 // Returns MOE_ERR_UNSUPPORTED (nothing enqueued) if the shape does not fit the tensor-core path.

@@ -20,6 +20,16 @@ struct FfnGroup {
   const int32_t* mtile;    // M-tile -> expert table (tensor-core path) or nullptr
   int row_align;
   int st_fwd1, st_fwd2, st_bwd1, st_bwd2, st_wgrad;  // profile stages of the five GEMM groups
+  // rows_fused(cfg) >= 1 (routed experts only): w (by flat position, rows mapped through gidx = perm_to_flat) is applied in
+  // the GEMM-1 / dgrad-down epilogues, so a holds w a and the copy called dy holds the UNWEIGHTED rows of dY;
+  // rows_fused(cfg) == 2: those two GEMMs also gather their A rows from the TOKEN-major tok_in (X / dY) themselves and
+  // write the row-grouped copies (Xp / dy) as a by-product
+  const int32_t* gidx = nullptr;
+  const void* tok_in = nullptr;
+  int gK = 1;
+  int64_t g_rows = 0;
+  const float* roww = nullptr;
+  float* dwpart = nullptr;
 };
 
 namespace {
@@ -57,6 +67,10 @@ int32_t ffn_fwd(const FfnGroup& g, const void* Xp, const void* Wg, const void* W
     TcCall c = tc_base(g, TC_FWD_SWIGLU);   // gu = [Xp Wg^T | Xp Wu^T], a = silu(g) * u
     c.A = Xp; c.lda = g.H; c.B0 = Wg; c.B1 = Wu; c.b_rows = g.F; c.b_cols = g.H; c.N = g.F; c.Kd = g.H;
     c.out0 = gu; c.ld0 = 2 * g.F; c.out1 = a; c.ld1 = g.F;
+    if (g.gidx) { c.gidx = g.gidx; c.roww = g.roww; }   // a = w silu(g) u
+    if (g.tok_in) {                         // A = X [T,H] gathered in the kernel; Xp is its by-product
+      c.A = g.tok_in; c.gat = 1; c.gK = g.gK; c.g_rows = g.g_rows; c.copy_out = const_cast<void*>(Xp); c.ld_copy = g.H;
+    }
     MOE_CHECK(tc_gemm(c, s));
     prof_mark(g.st_fwd1, s);
     c = tc_base(g, TC_FWD);                 // y = a Wd^T
@@ -116,6 +130,10 @@ int32_t ffn_bwd(const FfnGroup& g, const void* dy, const void* Xp, const void* g
     TcCall c = tc_base(g, TC_DGRAD_SWIGLU);   // dgu = swiglu'(gu) * (dy Wd[e])
     c.A = dy; c.lda = g.H; c.B0 = Wd; c.b_rows = g.H; c.b_cols = g.F; c.N = g.F; c.gu = gu; c.ldgu = 2 * g.F;
     c.out0 = dgu; c.ld0 = 2 * g.F;
+    if (g.gidx) { c.gidx = g.gidx; c.roww = g.roww; c.dwpart = g.dwpart; }   // dgu = w swiglu'(gu) da; dwpart = <da, a>
+    if (g.tok_in) {                           // A = dY [T,H] gathered in the kernel; dy = its unweighted by-product copy
+      c.A = g.tok_in; c.gat = 1; c.gK = g.gK; c.g_rows = g.g_rows; c.copy_out = const_cast<void*>(dy); c.ld_copy = g.H;
+    }
     MOE_CHECK(tc_gemm(c, s));
     prof_mark(g.st_bwd1, s);
     c = tc_base(g, TC_DGRAD);                 // dXp = dg Wg[e] + du Wu[e]: one contraction over [dg|du]
@@ -292,12 +310,15 @@ extern "C" int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, cons
   prof_mark(ST_ROUTE, s);
   MOE_CHECK(build_maps(cfg, topk_idx, counts, offsets, p2f, f2p, mtile, at<int32_t>(ws, W.hist), s));  // R6
   prof_mark(ST_MAPS, s);
-  MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, Xp, s));
+  const int fused = rows_fused(cfg);       // 2: X is gathered inside GEMM-1, which also writes Xp: no permute pass
+  if (fused < 2) MOE_CHECK(gather_rows(cfg, X, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, Xp, s));
   prof_mark(ST_PERMUTE, s);
   // the FFN runs over the experts that own weights (all of them unless zero-computation experts are configured, V2)
   FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  if (fused) { g.gidx = p2f; g.gK = cfg->K; g.g_rows = cfg->T; g.roww = topk_w; }
+  if (fused == 2) g.tok_in = X;
   Fp8Bufs q, qs;
   memset(&q, 0, sizeof(q));
   memset(&qs, 0, sizeof(qs));
@@ -342,7 +363,8 @@ extern "C" int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, cons
       MOE_CHECK(ffn_fwd(gs, X, Wg_s, Wu_s, Wd_s, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
     shared_out = at<char>(ctx, C.y_s);
   }
-  MOE_CHECK(combine(cfg, y, topk_w, f2p, shared_out, nullptr, nullptr, nullptr, nullptr, Y, s));    // R7 combine
+  // R7 combine (fused rows: y already carries w, so a plain sum over the K rows)
+  MOE_CHECK(combine(cfg, y, fused ? nullptr : topk_w, f2p, shared_out, nullptr, nullptr, nullptr, nullptr, Y, s));
   prof_mark(ST_COMBINE, s);
   return MOE_OK;
 }
@@ -395,11 +417,17 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
   void* tmp = at<char>(ws, W.tmp);
 
   prof_mark(ST_BEGIN, s);
-  MOE_CHECK(combine_bwd(cfg, dY, y, w, f2p, p2f, offsets, dy, dw, s));                     // R8 combine-bwd
+  // fused rows: no combine-bwd pass (no read of y): dy = the UNWEIGHTED rows of dY (a plain gather, or with 2 the by-product
+  // of dgrad-down's own gather); dgrad-down applies w and produces dw in its epilogue
+  const int fused = rows_fused(cfg);
+  if (!fused) MOE_CHECK(combine_bwd(cfg, dY, y, w, f2p, p2f, offsets, dy, dw, s));         // R8 combine-bwd
+  if (fused == 1) MOE_CHECK(gather_rows(cfg, dY, cfg->H, elem_bytes(cfg), f2p, p2f, offsets, dy, s));
   prof_mark(ST_COMBINE_BWD, s);
   FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  if (fused) { g.gidx = p2f; g.gK = cfg->K; g.g_rows = cfg->T; g.roww = w; g.dwpart = at<float>(ws, W.dwpart); }
+  if (fused == 2) g.tok_in = dY;
   Fp8Bufs q, qs;
   memset(&q, 0, sizeof(q));
   memset(&qs, 0, sizeof(qs));
@@ -427,6 +455,10 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
     MOE_CHECK(ffn_bwd_fp8(g, q, dy, Xp, gu, a, dgu, dXp, dWg, dWu, dWd, s));               // R8 expert FFN on the codes
   } else {
     MOE_CHECK(ffn_bwd(g, dy, Xp, gu, a, Wg, Wu, Wd, tmp, dgu, dXp, dWg, dWu, dWd, s));     // R8 expert FFN
+    if (fused) {
+      MOE_CHECK(dw_reduce(cfg, g.dwpart, 2 * (int)ceil_div(cfg->F, 256), f2p, dw, s));     // dw[t,j] = <da_r, a_r>
+      prof_mark(ST_COMBINE_BWD, s);
+    }
   }
   MOE_CHECK(zc_backward(cfg, offsets, counts, dy, dgu, dXp, ex ? ex->d_zc_const : nullptr, s));      // V2: dXp = 0 | dy | 0
   const bool dense = dense_router_bwd(cfg);
@@ -435,8 +467,8 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
                                offsets + cfg->E + 1, dz, at<float>(ws, W.dzd), at<char>(ws, W.dzb), dWr, at<char>(ws, W.dXr),
                                s));
   else
-    MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr, Xp, dz,
-                         dzp, at<float>(ws, W.dwr_part), dWr, s));                                    // R8 router
+    MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr,
+                         Xp, dz, dzp, at<float>(ws, W.dwr_part), dWr, s));                                    // R8 router
   prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
   if (shared) {

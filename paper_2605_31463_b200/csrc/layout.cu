@@ -1,4 +1,5 @@
 // Config validation, ctx / ws byte layouts and the small query entry points of the C ABI.
+#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -38,6 +39,14 @@ int32_t layer_preflight(const moe_config_t* c, bool backward) {
   if (c->dtype == 2 && c->row_align % 128 != 0) return MOE_ERR_UNSUPPORTED;
   (void)backward;
   return MOE_OK;
+}
+
+int rows_fused(const moe_config_t* c) {
+  const bool ok = c->dtype == 1 && c->H % 64 == 0 && c->F % 64 == 0 && c->row_align % 128 == 0 && n_zc(c) == 0;
+  if (!ok) return 0;
+  const char* e = getenv("MOE_B200_FUSED_ROWS");      // read per call: tests flip it inside one process
+  if (e && e[0] >= '0' && e[0] <= '2') return e[0] - '0';
+  return 1;
 }
 
 int device_sm_count() {
@@ -125,7 +134,8 @@ WsLayout ws_layout(const moe_config_t* c) {
   L.dz = k.take(T * c->K * 4);
   L.dzp = k.take(R * 4);
   L.dwr_part = k.take((R / 128 + 1) * H * 4);   // per-tile partial sums of dWr (fp32)
-  L.dy = k.take(R * H * es);
+  L.dy = k.take(R * H * es);                                 // fused rows: the UNWEIGHTED gathered dY
+  if (rows_fused(c)) L.dwpart = k.take(2 * ((F + 255) / 256) * R * 4);
   L.dgu = k.take(R * 2 * F * es);
   L.dXp = k.take(R * H * es);
   if (Fs) {
@@ -167,6 +177,11 @@ extern "C" const char* moe_status_string(int32_t status) {
 extern "C" int32_t moe_version(void) { return 100; }
 
 extern "C" int64_t moe_launch_count(void) { return g_launches; }
+
+extern "C" int32_t moe_layer_rows_fused(const moe_config_t* cfg) {
+  if (validate(cfg) != MOE_OK) return MOE_ERR_INVALID_ARG;
+  return rows_fused(cfg);
+}
 
 extern "C" int64_t moe_padded_rows(const moe_config_t* cfg) {
   if (validate(cfg) != MOE_OK) return -1;

@@ -239,7 +239,26 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_bwd_kernel(const int4*
   }
 }
 
+// dw[p] = sum_k part[k, f2p[p]] in ascending k (deterministic); an empty slot (f2p < 0) gets 0.
+__global__ void __launch_bounds__(256) dw_reduce_kernel(const float* __restrict__ part, int nparts, int64_t R,
+                                                        const int32_t* __restrict__ f2p, int64_t TK,
+                                                        float* __restrict__ dw) {
+  const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= TK) return;
+  const int r = f2p[i];
+  float s = 0.f;
+  if (r >= 0)
+    for (int k = 0; k < nparts; ++k) s += part[(int64_t)k * R + r];
+  dw[i] = s;
+}
+
 }  // namespace
+
+int32_t dw_reduce(const moe_config_t* c, const float* part, int nparts, const int32_t* f2p, float* dw, cudaStream_t s) {
+  const int64_t TK = (int64_t)c->T * c->K;
+  MOE_LAUNCH(dw_reduce_kernel, (unsigned)ceil_div(TK, 256), 256, 0, s, part, nparts, padded_rows(c), f2p, TK, dw);
+  return MOE_OK;
+}
 
 int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, const int32_t* f2p, const int32_t* p2f,
                     const int32_t* offsets, void* Xp, cudaStream_t s) {

@@ -102,6 +102,12 @@ def check_routing_replay(cfg, z_gpu, bias, idx_gpu, w_gpu, z_truth=None, thresho
     return 0
 
 
+def row_weights(p2f, w):
+    """Routing weight of every permuted row (0 for padding rows): w.reshape(-1)[perm_to_flat]."""
+    p2f = np.asarray(p2f, np.int64)
+    return np.where(p2f >= 0, np.asarray(w, np.float64).reshape(-1)[np.maximum(p2f, 0)], 0.0)
+
+
 def compare_layer(cfg, inp, lb, backward=True, tol=None):
     """Oracle on the same inputs with the GPU's (replay-verified) selection; returns the error table."""
     from paper_2605_31463_b200.buffers import to_numpy
@@ -122,12 +128,14 @@ def compare_layer(cfg, inp, lb, backward=True, tol=None):
     R = int(fwd["offsets"][-1])
     assert np.array_equal(to_numpy(lb.ctx_view("perm_to_flat"))[:R], fwd["perm_to_flat"])
     assert orc.rel_fro(w_gpu, fwd["w"]) <= TOL_ROUTER
-    if cfg.dtype != wl.DTYPE_FP8:
+    if cfg.dtype != wl.DTYPE_FP8:      # fused rows: Xp is GEMM-1's by-product copy of its gathered tiles
         assert np.array_equal(to_numpy(lb.ctx_view("Xp"))[:R], fwd["Xp"].astype(np.float32)), "Xp must be a bit-exact copy"
+    # fused rows (moe_layer_rows_fused): the saved a and y carry the row's routing weight, padding rows stay zero
+    wrow = row_weights(fwd["perm_to_flat"], fwd["w"]) if lb.rows_fused else np.ones(R)
     gu = to_numpy(lb.ctx_view("gu"))[:R]
     acts = [("g", gu[:, :cfg.F], fwd["g"]), ("u", gu[:, cfg.F:], fwd["u"]),
-            ("a", to_numpy(lb.ctx_view("a"))[:R], fwd["a"]), ("y", to_numpy(lb.ctx_view("y"))[:R], fwd["y"]),
-            ("Y", to_numpy(lb.Y), fwd["Y"])]
+            ("a", to_numpy(lb.ctx_view("a"))[:R], fwd["a"] * wrow[:, None]),
+            ("y", to_numpy(lb.ctx_view("y"))[:R], fwd["y"] * wrow[:, None]), ("Y", to_numpy(lb.Y), fwd["Y"])]
     if cfg.aux_coef:                                             # A1..A2: loss value, f, P (fp32 router-side quantities)
         errs["aux_loss"] = abs(float(to_numpy(lb.aux_loss)[0]) - fwd["aux_loss"]) / abs(fwd["aux_loss"])
         assert errs["aux_loss"] <= TOL_ROUTER, errs["aux_loss"]
@@ -137,6 +145,10 @@ def compare_layer(cfg, inp, lb, backward=True, tol=None):
         del errs["aux_loss"]
     if backward:
         bwd = orc.layer_bwd(cfg, inp["dY"], inp["X"], inp["Wr"], inp["W"], fwd, inp["shared"], extras=ex)
+        if lb.rows_fused:              # ws "dy": dgrad-down's by-product copy of the gathered dY rows, unweighted, zero padding
+            p2f = np.asarray(fwd["perm_to_flat"], np.int64)
+            dyp = np.where((p2f >= 0)[:, None], inp["dY"].astype(np.float32)[np.maximum(p2f, 0) // cfg.K], 0.0)
+            assert np.array_equal(to_numpy(lb.ws_view("dy"))[:R], dyp), "gathered dY must be a bit-exact copy"
         errs["dw"] = orc.rel_fro(to_numpy(lb.ws_view("dw")), bwd["dw"])
         errs["dWr"] = orc.rel_fro(to_numpy(lb.dWr), bwd["dWr"])
         dgu = to_numpy(lb.ws_view("dgu"))[:R]

@@ -109,7 +109,8 @@ def test_full_size_sampled_outputs(cfg0):
         else:
             dXp, dWg, dWu, dWd, dg, du = orc.expert_ffn_bwd(dy, X64[tok], g, u, a, *W3)
         note("g", orc.rel_fro(to_numpy(gu_g[sl, :F]), g)); note("u", orc.rel_fro(to_numpy(gu_g[sl, F:]), u))
-        note("a", orc.rel_fro(to_numpy(a_g[sl]), a)); note("y", orc.rel_fro(to_numpy(y_g[sl]), y))
+        ws_ = wr[:, None] if lb.rows_fused else 1.0          # fused rows: the saved a, y carry the routing weight
+        note("a", orc.rel_fro(to_numpy(a_g[sl]), a * ws_)); note("y", orc.rel_fro(to_numpy(y_g[sl]), y * ws_))
         note("dg", orc.rel_fro(to_numpy(dgu_g[sl, :F]), dg)); note("du", orc.rel_fro(to_numpy(dgu_g[sl, F:]), du))
         note("dXp", orc.rel_fro(to_numpy(dXp_g[sl]), dXp))
         note("dWg", orc.rel_fro(to_numpy(lb.dWg[e]), dWg)); note("dWu", orc.rel_fro(to_numpy(lb.dWu[e]), dWu))

@@ -182,3 +182,36 @@ def test_pipelined_host_step_matches_device_step():
     torch.cuda.synchronize()
     for i in range(n):
         assert torch.equal(Yh[i], refs[i % 2].Y.cpu()) and torch.equal(dXh[i], refs[i % 2].dX.cpu()), i
+
+
+FUSED_CASES = [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128),
+               wl.DSV3_SMALL.replace(name="dsv3_small_align128", row_align=128),
+               wl.GPTOSS_SMALL.replace(name="gptoss_small_align128", row_align=128)]
+
+
+@pytest.mark.parametrize("level", [0, 2])
+@pytest.mark.parametrize("cfg", FUSED_CASES, ids=lambda c: c.name)
+def test_other_fusion_levels_match_oracle(cfg, level, monkeypatch):
+    """bf16 layers default to moe_layer_rows_fused = 1 (routing weight in the GEMM-1 / dgrad-down epilogues, dw from the
+    dgrad-down epilogue; covered by test_layer_fwd_bwd_matches_oracle).  MOE_B200_FUSED_ROWS=0 keeps w in the combine and
+    the combine-backward pass, =2 also gathers the rows of X / dY inside the GEMMs (TMA tile::gather4) with Xp / dy as
+    by-product copies: same oracle, same tolerance, and all three agree on the routing bit for bit."""
+    import torch
+    inp = gc.gen_inputs(cfg)
+    dflt = gc.run_gpu_layer(cfg, inp)
+    assert dflt.rows_fused == 1
+    monkeypatch.setenv("MOE_B200_FUSED_ROWS", str(level))
+    lb = gc.run_gpu_layer(cfg, inp)
+    assert lb.rows_fused == level
+    errs = gc.compare_layer(cfg, inp, lb)
+    assert torch.equal(lb.topk_idx, dflt.topk_idx) and torch.equal(lb.topk_w, dflt.topk_w)
+    print(cfg.name, "fusion level", level, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
+
+
+def test_fused_rows_query():
+    import paper_2605_31463_b200 as moe
+    assert moe.moe_layer_rows_fused(wl.QWEN3_SMALL.replace(row_align=128)) == 1
+    # fp32, unaligned groups and FP8 keep w in the combine and the combine-backward pass
+    assert moe.moe_layer_rows_fused(wl.TINY) == 0
+    assert moe.moe_layer_rows_fused(wl.QWEN3_SMALL) == 0
+    assert moe.moe_layer_rows_fused(wl.DSV3_FP8_SMALL.replace(row_align=128)) == 0
