@@ -130,7 +130,8 @@ int32_t route_impl(const moe_config_t* c, const float* logits, const float* bias
 int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, float* z, cudaStream_t s);
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
                    const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const int32_t* mtile,
-                   const void* Xp, float* dz, float* dzp, float* part, void* dWr, cudaStream_t s);
+                   const void* Xp, const void* X /* token-major, with p2f: read instead of Xp; or NULL */, const int32_t* p2f,
+                   float* dz, float* dzp, float* part, void* dWr, cudaStream_t s);
 // dense router backward (A3 / softmax without renorm / V2): dz [T,E] fp32 (+ bf16 copy), dWr = dz^T X, dXr = dz Wr
 int32_t router_bwd_dense(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
                          const float* aux_f, const void* X, const void* Wr, const int32_t* off_one /* device {0, T} */,

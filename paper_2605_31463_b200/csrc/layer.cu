@@ -468,7 +468,7 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
                                s));
   else
     MOE_CHECK(router_bwd(cfg, z, idx, w, dw, f2p, offsets, counts, (cfg->row_align % 128 == 0) ? mtile : nullptr,
-                         Xp, dz, dzp, at<float>(ws, W.dwr_part), dWr, s));                                    // R8 router
+                         Xp, X, p2f, dz, dzp, at<float>(ws, W.dwr_part), dWr, s));                                    // R8 router
   prof_mark(ST_ROUTER_BWD, s);
   const void* dXs = nullptr;
   if (shared) {

@@ -132,7 +132,10 @@ __global__ void __launch_bounds__(256) dwr_tile_kernel(const float* __restrict__
                                                        const int32_t* __restrict__ mtile,
                                                        const int32_t* __restrict__ offsets,
                                                        const int32_t* __restrict__ counts, int H,
+                                                       const int32_t* __restrict__ p2f, int K,
                                                        float* __restrict__ part) {
+  // p2f != nullptr: Xp is the TOKEN-major X [T,H] and permuted row r reads token row p2f[r] / K -- X (T H bytes) stays in
+  // L2 across the K experts that touch each row, the row-grouped copy (K times larger) would stream from HBM
   __shared__ float red[8][256];
   const int tile = blockIdx.x;
   if (tile >= mtile[0]) return;
@@ -150,7 +153,8 @@ __global__ void __launch_bounds__(256) dwr_tile_kernel(const float* __restrict__
       const int r = r0 + i;
       if (r >= live_end) break;
       const float d = dzp[r];
-      const uint4 v = __ldg(Xp + ((size_t)r * H + col) / 8);
+      const size_t src = p2f ? (size_t)(p2f[r] / K) : (size_t)r;          // live rows only: p2f[r] >= 0
+      const uint4 v = __ldg(Xp + (src * H + col) / 8);
       const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
@@ -473,14 +477,16 @@ int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, floa
 
 int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, const float* w, const float* dw,
                    const int32_t* f2p, const int32_t* offsets, const int32_t* counts, const int32_t* mtile,
-                   const void* Xp, float* dz, float* dzp, float* part, void* dWr, cudaStream_t s) {
+                   const void* Xp, const void* X, const int32_t* p2f, float* dz, float* dzp, float* part, void* dWr,
+                   cudaStream_t s) {
   if (c->score_fn == 0 && !c->renorm) return MOE_ERR_UNSUPPORTED;  // dense dz: not on any config's path
   MOE_LAUNCH(dz_kernel, (unsigned)ceil_div(c->T, 4), 128, 0, s, z, idx, w, dw, f2p, c->T, c->E, c->K, c->score_fn,
              c->renorm, c->routed_scale, dz, dzp);
   if (dWr && c->dtype != 0 && c->row_align % 128 == 0 && c->H % 8 == 0 && mtile && part) {
     const unsigned slabs = (unsigned)ceil_div(c->H, 256);
-    MOE_LAUNCH(dwr_tile_kernel, dim3((unsigned)(padded_rows(c) / 128), slabs), 256, 0, s, dzp, (const uint4*)Xp, mtile,
-               offsets, counts, c->H, part);
+    const bool tok = X != nullptr && p2f != nullptr;     // read the token-major X through the map
+    MOE_LAUNCH(dwr_tile_kernel, dim3((unsigned)(padded_rows(c) / 128), slabs), 256, 0, s, dzp, (const uint4*)(tok ? X : Xp),
+               mtile, offsets, counts, c->H, tok ? p2f : nullptr, c->K, part);
     MOE_LAUNCH(dwr_reduce_kernel, dim3((unsigned)c->E, slabs), 256, 0, s, part, offsets, c->H, (__nv_bfloat16*)dWr);
   } else if (dWr) {
     dim3 grid((unsigned)c->E, (unsigned)ceil_div(c->H, 256));

@@ -1,6 +1,8 @@
 // Row movers on the permutation maps: gather (moe_permute), weighted combine (moe_unpermute_combine,
 // also the dX reduction) and combine-backward.  SURVEY.md §8c R6/R7/R8.  All HBM-bound: one warp per
 // token, 16-byte vector accesses, each source row read once, fixed j order, fp32 accumulation.
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace moe {
@@ -8,6 +10,7 @@ namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int ROW_WARPS = 8;
+constexpr int COMBINE_CTAS = 4096; // aim of the combine's grid: about seven waves of 4 resident CTAs per SM
 
 __device__ __forceinline__ int4 ldg_stream(const int4* p) {
   int4 r;
@@ -32,7 +35,8 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
   if (t >= T) return;
   const int4* src = X + (size_t)t * nvec;
   const int32_t* rows = f2p + (size_t)t * K;
-  for (int v0 = 0; v0 < nvec; v0 += 128) {
+  // blockIdx.y = 2 KB column slab of the row: enough CTAs for several waves even when T / 8 is about one wave
+  for (int v0 = blockIdx.y * 128; v0 < min(nvec, (int)(blockIdx.y + 1) * 128); v0 += 128) {
     int4 buf[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -52,15 +56,17 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
   }
 }
 
-// Zero the padding rows (perm_to_flat[r] < 0) below offsets[E]: one warp per row, every row's map entry read in parallel.
+// Zero the padding rows of every expert group: they are the tail of the group (perm_to_flat[r] < 0), at most row_align - 1
+// rows.  One CTA per expert, one warp per row, walking up from the group's end until a real row is met.
 __global__ void __launch_bounds__(ROW_WARPS * 32) zero_pad_kernel(const int32_t* __restrict__ p2f,
-                                                                   const int32_t* __restrict__ offsets, int E,
-                                                                   int nvec, int64_t rows_cap, int4* __restrict__ Xp) {
+                                                                   const int32_t* __restrict__ offsets, int nvec,
+                                                                   int4* __restrict__ Xp) {
   const int lane = threadIdx.x & 31;
-  const int64_t r = (int64_t)blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
-  if (r >= rows_cap || r >= offsets[E] || p2f[r] >= 0) return;
-  int4* dst = Xp + (size_t)r * nvec;
-  for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
+  const int begin = offsets[blockIdx.x], end = offsets[blockIdx.x + 1];
+  for (int r = end - 1 - (int)(threadIdx.x >> 5); r >= begin && p2f[r] < 0; r -= ROW_WARPS) {
+    int4* dst = Xp + (size_t)r * nvec;
+    for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
+  }
 }
 
 template <typename T>
@@ -107,14 +113,15 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
                                                                   const float* __restrict__ dz,
                                                                   const int32_t* __restrict__ idx,
                                                                   const int4* __restrict__ Wr, int Tn, int Krt, int nvec,
-                                                                  int4* __restrict__ Y) {
+                                                                  int slab, int4* __restrict__ Y) {
   constexpr int N = Vec<T>::N;
   const int K = KT > 0 ? KT : Krt;
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= Tn) return;
   const int32_t* rows = f2p + (size_t)t * K;
-  for (int v = lane; v < nvec; v += 32) {
+  // blockIdx.y = column slab of `slab` 16-byte vectors (a multiple of 32): several waves of CTAs whatever T is
+  for (int v = blockIdx.y * slab + lane; v < min(nvec, (int)(blockIdx.y + 1) * slab); v += 32) {
     float acc[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) acc[i] = 0.f;
@@ -265,8 +272,8 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
   if ((cols * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(cols * esz / 16);
 #define MOE_GATHER(KT)                                                                                              \
-  MOE_LAUNCH(gather_kernel<KT>, (unsigned)ceil_div(c->T, ROW_WARPS), ROW_WARPS * 32, 0, s, (const int4*)X, c->T, c->K, \
-             nvec, f2p, (int4*)Xp)
+  MOE_LAUNCH(gather_kernel<KT>, dim3((unsigned)ceil_div(c->T, ROW_WARPS), (unsigned)ceil_div(nvec, 128)), ROW_WARPS * 32, 0, s, \
+             (const int4*)X, c->T, c->K, nvec, f2p, (int4*)Xp)
   switch (c->K) {
     case 2: MOE_GATHER(2); break;
     case 4: MOE_GATHER(4); break;
@@ -274,9 +281,7 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
     default: MOE_GATHER(0); break;
   }
 #undef MOE_GATHER
-  if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, (unsigned)ceil_div(padded_rows(c), ROW_WARPS), ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec,
-               padded_rows(c), (int4*)Xp);
+  if (c->row_align > 1) MOE_LAUNCH(zero_pad_kernel, (unsigned)c->E, ROW_WARPS * 32, 0, s, p2f, offsets, nvec, (int4*)Xp);
   return MOE_OK;
 }
 
@@ -285,10 +290,17 @@ int32_t combine(const moe_config_t* c, const void* y, const float* w, const int3
   const size_t esz = elem_bytes(c);
   if ((c->H * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(c->H * esz / 16);
-  const unsigned grid = (unsigned)ceil_div(c->T, ROW_WARPS);
+  // Rows are cut into column slabs only when whole rows give fewer than ~3.5 waves of CTAs (4 resident per SM), where the
+  // ragged last wave costs more than the split: measured configs[1] (1024 CTAs) 85 -> 70 us, configs[2] (512) 165 -> 133 us
+  // with slabs, but configs[4] (2048 CTAs, 5.8 KB rows) 92 -> 108 us, so it keeps whole rows.
+  const int64_t base_ctas = ceil_div(c->T, ROW_WARPS);
+  const int slabs = base_ctas >= COMBINE_CTAS / 2
+                        ? 1 : (int)std::max<int64_t>(1, std::min<int64_t>(ceil_div(nvec, 64), COMBINE_CTAS / base_ctas));
+  const int slab = (int)round_up(ceil_div(nvec, slabs), 32);
+  const dim3 grid((unsigned)base_ctas, (unsigned)ceil_div(nvec, slab));
 #define MOE_COMBINE(TY, KT)                                                                                       \
   MOE_LAUNCH((combine_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, (const int4*)add1, dz, idx, \
-             (const int4*)Wr, c->T, c->K, nvec, (int4*)Y)
+             (const int4*)Wr, c->T, c->K, nvec, slab, (int4*)Y)
   if (c->dtype == 0) {
     MOE_COMBINE(float, 0);
   } else {
@@ -323,9 +335,7 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
     }
   }
 #undef MOE_COMBINE_BWD
-  if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, (unsigned)ceil_div(padded_rows(c), ROW_WARPS), ROW_WARPS * 32, 0, s, p2f, offsets, c->E, nvec,
-               padded_rows(c), (int4*)dy);
+  if (c->row_align > 1) MOE_LAUNCH(zero_pad_kernel, (unsigned)c->E, ROW_WARPS * 32, 0, s, p2f, offsets, nvec, (int4*)dy);
   return MOE_OK;
 }
 
