@@ -89,16 +89,20 @@ constexpr int B_BYTES = BN * BK * 2;   // 32 KB: all 256 columns of the right op
 // k-block costs each SM 32 KB of L2 -> SM traffic instead of 48 KB for the same 128 x 256 x 64 MACs; the 32 KB this
 // saves hold a second staging box per epilogue warp group (NOBUF), so a group fills one box while the TMA store of
 // its other box is still reading shared memory.
-template <bool PAIR> struct Ring {
-  static constexpr int STAGES = PAIR ? 5 : 4;
+// SHORT (1-CTA weight gradients): an expert's contraction is a handful of k-blocks and every tile ends with 64 KB of output,
+// so a stage of the ring is traded for a second staging box per warp group (3 stages, NOBUF 2).
+template <bool PAIR, bool SHORT = false> struct Ring {
+  static constexpr int STAGES = PAIR ? 5 : (SHORT ? 3 : 4);
   static constexpr int B_CTA = PAIR ? B_BYTES / 2 : B_BYTES;
   static constexpr int STAGE_BYTES = A_BYTES + B_CTA;
-  static constexpr int NOBUF = PAIR ? 2 : 1;   // staging boxes per epilogue warp group
+  static constexpr int NOBUF = (PAIR || SHORT) ? 2 : 1;   // staging boxes per epilogue warp group
 };
 constexpr int MAX_STAGES = 6;
 constexpr int MN_BOX_BYTES = 64 * BK * 2;  // one 64(MN) x 64(K) box of an MN-major operand: 8 KB
 constexpr int OBUF_BYTES = BM * 128;       // epilogue staging: 128 rows x 64 bf16 columns (one 128-byte-swizzled TMA box)
 constexpr int SMEM_BYTES = Ring<false>::STAGES * Ring<false>::STAGE_BYTES + 2 * OBUF_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+static_assert(Ring<false, true>::STAGES * Ring<false, true>::STAGE_BYTES + 2 * Ring<false, true>::NOBUF * OBUF_BYTES <=
+              Ring<false>::STAGES * Ring<false>::STAGE_BYTES + 2 * Ring<false>::NOBUF * OBUF_BYTES, "fits the same allocation");
 static_assert(Ring<true>::STAGES * Ring<true>::STAGE_BYTES + 2 * Ring<true>::NOBUF * OBUF_BYTES ==
               Ring<false>::STAGES * Ring<false>::STAGE_BYTES + 2 * Ring<false>::NOBUF * OBUF_BYTES, "same shared-memory footprint");
 constexpr int EPI_WARPS = 8;            // two per TMEM lane group: column-chunk parity `ch` splits a tile between them
@@ -109,7 +113,7 @@ constexpr int TMEM_COLS = 512;
 // kernel parameters
 // ---------------------------------------------------------------------------------------------
 struct TcParams {
-  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, tma_out, acc_f32;
+  int E, n_tiles, m_tiles, nkb, kb_split, b_rows, N, M, F, a_col0, tma_out, acc_f32, short_ring;
   int64_t rows_valid;
   const int32_t* mtile;    // M-tile -> expert (nullptr: one group of rows_valid rows)
   const int32_t* tlist;    // which M-tiles this launch runs: pair kernel = plist, 1-CTA kernel = olist or nullptr (all)
@@ -563,8 +567,13 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                const __grid_constant__ CUtensorMap tmO2, const __grid_constant__ CUtensorMap tmC, const TcParams p) {
   constexpr bool A_MN = (MODE == TC_WGRAD);
   constexpr bool B_MN = (MODE == TC_DGRAD || MODE == TC_DGRAD_SWIGLU || MODE == TC_WGRAD);
-  constexpr int STAGES = Ring<PAIR>::STAGES, STAGE_BYTES = Ring<PAIR>::STAGE_BYTES, B_CTA = Ring<PAIR>::B_CTA;
-  constexpr int NOBUF = Ring<PAIR>::NOBUF, GROUP_OBUF = NOBUF * OBUF_BYTES;   // staging bytes of one epilogue warp group
+  using R = Ring<PAIR>;
+  constexpr int STAGE_BYTES = R::STAGE_BYTES, B_CTA = R::B_CTA;
+  // the 1-CTA weight-gradient kernel picks its ring at run time (p.short_ring): 3 stages + 2 staging boxes per warp group
+  const bool short_ring = MODE == TC_WGRAD && !PAIR && p.short_ring;
+  const int STAGES = short_ring ? Ring<false, true>::STAGES : R::STAGES;
+  const int NOBUF = short_ring ? Ring<false, true>::NOBUF : R::NOBUF;
+  const int GROUP_OBUF = NOBUF * OBUF_BYTES;   // staging bytes of one epilogue warp group
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128-byte swizzle wants 1024-byte alignment
   const uint32_t obuf0 = base + STAGES * STAGE_BYTES;
@@ -584,7 +593,7 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     tma_prefetch_desc(&tmB1);
     tma_prefetch_desc(&tmO);
     tma_prefetch_desc(&tmO2);
-    for (int s = 0; s < STAGES; ++s) {
+    for (int s = 0; s < MAX_STAGES; ++s) {
       mbar_init(full0 + 8 * s, 1);
       mbar_init(empty0 + 8 * s, (GW > 0 && p.copy_out) ? 2 : 1);   // MMA commit (+ the copy-out warp's store has read the stage)
     }
@@ -770,10 +779,17 @@ tc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         // the accumulator is released inside, right after its last TMEM load (one arrive per warp)
         auto rel = [&]() { if (have) release_acc(as); };
         if (MODE == TC_WGRAD && p.acc_f32) {
-          if (have) wgrad_accum_tile<NOBUF>(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch, oseq, rel);
+          if (have) {
+            if (NOBUF == 2) wgrad_accum_tile<2>(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch, oseq, rel);
+            else wgrad_accum_tile<1>(p, tl, tacc, row_in_tile, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch, oseq, rel);
+          }
         } else {
-          wgrad_store_tile<NOBUF>(p, tl, tacc, row_in_tile, have, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch,
-                                  MODE == TC_WGRAD ? tl.e : 0, oseq, rel);
+          if (NOBUF == 2)
+            wgrad_store_tile<2>(p, tl, tacc, row_in_tile, have, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch,
+                                MODE == TC_WGRAD ? tl.e : 0, oseq, rel);
+          else
+            wgrad_store_tile<1>(p, tl, tacc, row_in_tile, have, obuf0 + ch * GROUP_OBUF, &tmO, (threadIdx.x & 127) == 64, ch,
+                                MODE == TC_WGRAD ? tl.e : 0, oseq, rel);
         }
         if (have && ++as == 2) { as = 0; aphase ^= 1; }
         continue;
@@ -1108,6 +1124,10 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
                     : !tc_make_map3(&to, 2, c.out0, c.N, c.M, c.E, c.ld0, 64, BM))   // bf16 dB [E, M, N], overwrite
         return MOE_ERR_UNSUPPORTED;
       const int64_t units = (int64_t)c.E * p.m_tiles * p.n_tiles;
+      // short contractions (about 256 real rows per expert or fewer): every tile is mostly its 64 KB of output, so the
+      // 1-CTA kernel trades a ring stage for a second staging box per warp group (configs[2]: 7.30 -> 6.73 ms; with the
+      // long contractions of configs[4] the 4-stage ring is 2 % faster)
+      p.short_ring = (c.mtile != nullptr && c.rows_cap < 384 * (int64_t)c.E) ? 1 : 0;
       if (pair) return launch<TC_WGRAD, true>(ta, tb0, tb0, to, p, units, s);
       return launch<TC_WGRAD, false>(ta, tb0, tb0, to, p, units, s);
     }

@@ -105,7 +105,7 @@ struct Vec<__nv_bfloat16> {
 
 // Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t]) (+ add1[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
 // Empty slots (f2p = -1, variable-k routing) contribute nothing.
-template <typename T, int KT>
+template <typename T, int KT, bool SLABBED>
 __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
                                                                   const int32_t* __restrict__ f2p,
                                                                   const int4* __restrict__ add0,
@@ -120,8 +120,10 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __r
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= Tn) return;
   const int32_t* rows = f2p + (size_t)t * K;
-  // blockIdx.y = column slab of `slab` 16-byte vectors (a multiple of 32): several waves of CTAs whatever T is
-  for (int v = blockIdx.y * slab + lane; v < min(nvec, (int)(blockIdx.y + 1) * slab); v += 32) {
+  // SLABBED: blockIdx.y = column slab of `slab` 16-byte vectors (a multiple of 32); else whole rows
+  const int v0 = SLABBED ? (int)blockIdx.y * slab : 0;
+  const int v1 = SLABBED ? min(nvec, v0 + slab) : nvec;
+  for (int v = v0 + lane; v < v1; v += 32) {
     float acc[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) acc[i] = 0.f;
@@ -299,8 +301,14 @@ int32_t combine(const moe_config_t* c, const void* y, const float* w, const int3
   const int slab = (int)round_up(ceil_div(nvec, slabs), 32);
   const dim3 grid((unsigned)base_ctas, (unsigned)ceil_div(nvec, slab));
 #define MOE_COMBINE(TY, KT)                                                                                       \
-  MOE_LAUNCH((combine_kernel<TY, KT>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0, (const int4*)add1, dz, idx, \
-             (const int4*)Wr, c->T, c->K, nvec, slab, (int4*)Y)
+  do {                                                                                                            \
+    if (slabs > 1)                                                                                                \
+      MOE_LAUNCH((combine_kernel<TY, KT, true>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0,        \
+                 (const int4*)add1, dz, idx, (const int4*)Wr, c->T, c->K, nvec, slab, (int4*)Y);                  \
+    else                                                                                                          \
+      MOE_LAUNCH((combine_kernel<TY, KT, false>), grid, ROW_WARPS * 32, 0, s, (const int4*)y, w, f2p, (const int4*)add0,       \
+                 (const int4*)add1, dz, idx, (const int4*)Wr, c->T, c->K, nvec, slab, (int4*)Y);                  \
+  } while (0)
   if (c->dtype == 0) {
     MOE_COMBINE(float, 0);
   } else {
