@@ -59,7 +59,7 @@ def pick_config(name):
     if cfg is None:
         raise SystemExit(f"unknown config {name}; have {sorted(wl.CONFIGS) + sorted(wl.SMALL_CONFIGS)}")
     if cfg.dtype != wl.DTYPE_FP32:
-        cfg = cfg.replace(row_align=128)   # tensor-core path: expert groups start at multiples of 128 rows
+        cfg = cfg.replace(row_align=int(os.environ.get("MOE_BENCH_ROW_ALIGN", "128")))   # tensor-core path: expert groups start at multiples of 128 rows
     return cfg
 
 
@@ -214,6 +214,31 @@ def stage_bytes(cfg):
             "dgrad_down_swiglu": TK * H * ab + sc(TK, H) + W * ab + TK * 2 * F * b + TK * 2 * F * b,   # dy, Wd, gu -> dgu
             "dgrad_gateup": TK * 2 * F * ab + sc(TK, 2 * F) + 2 * W * ab + TK * H * b,   # dgu, Wg, Wu -> dXp
             "wgrad": TK * (2 * H + 3 * F) * b + 3 * W * b}                               # dy, a, dgu, Xp -> dWd, dWg, dWu
+
+
+def stage_write_bytes(cfg):
+    """The WRITTEN part of stage_bytes for the GEMM stages (results only)."""
+    b = 4 if cfg.dtype == wl.DTYPE_FP32 else 2
+    T, H, E, K, F, TK = cfg.T, cfg.H, cfg.E, cfg.K, cfg.F, cfg.T * cfg.K
+    return {"gemm1_swiglu": TK * 3 * F * b, "gemm2": TK * H * b, "dgrad_down_swiglu": TK * 2 * F * b, "dgrad_gateup": TK * H * b,
+            "wgrad": 3 * E * H * F * b}
+
+
+def measure_write_bandwidth(stream):
+    """Write-only HBM bandwidth of this GPU in GB/s (a 2 GiB device fill, median of 5): MEASURED_PEAKS.json holds a COPY
+    bandwidth (half reads, half writes); a stage that mostly writes (the weight gradients of configs[2]: 22.5 GB out) is
+    bounded by this lower figure instead."""
+    import torch
+    buf = torch.empty(2 << 30, dtype=torch.uint8, device="cuda")
+    ts = []
+    for i in range(7):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); buf.fill_(i); e1.record(stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            ts.append(e0.elapsed_time(e1))
+    del buf
+    return (2 << 30) / (sorted(ts)[len(ts) // 2] * 1e-3) / 1e9
 
 
 def roof(flops, byts, sec, peak_tflops, peak_gbs):
@@ -406,6 +431,7 @@ def run_cuda(args, cfg):
            "serial_ms_per_step": ms_serial / args.steps}
 
     standalone = time_standalone_movers(moe, lb, cfg, stream) if rank == 0 else None
+    write_gbs = measure_write_bandwidth(stream) if rank == 0 else None
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -418,7 +444,8 @@ def run_cuda(args, cfg):
     burst = (ms * 1e-3 < 1.0) or bool(clocks["sm_mhz"] and clocks["sm_max_mhz"] and clocks["sm_mhz"] > 0.9 * clocks["sm_max_mhz"])
     regime = "burst" if burst else "sustained"
     bf16_peak = peaks["bf16_burst"] if burst else peaks["bf16_sustained"]
-    sf, sb = stage_flops(cfg), stage_bytes(cfg)
+    sf, sb, swb = stage_flops(cfg), stage_bytes(cfg), stage_write_bytes(cfg)
+    peaks["hbm_write_gbs_measured_live"] = write_gbs
     if lb.rows_fused == 1:     # the combine-bwd slot holds a plain gather of dY (+ the dw reduction): permute's bytes
         sb["combine_bwd"] = sb["permute"]
     elif lb.rows_fused == 2:   # no permute / combine-bwd pass inside the layer: the slots hold only the dw reduction
@@ -444,6 +471,8 @@ def run_cuda(args, cfg):
             st["frac_nominal_hbm"] = st["gbs"] / NOMINAL["hbm_gbs"]
         if name in sf and name in sb and sf[name] and sec > 0:
             st["bound"], st["frac_of_binding_roof"] = roof(sf[name], sb[name], sec, stage_peak(name), peaks["hbm_gbs"])
+        if name in swb and sec > 0:     # the write roof: results only, against the write-only bandwidth measured in this run
+            st["frac_hbm_write_roof"] = swb[name] / (write_gbs * 1e9) / sec
     gemm_stages = [n for n in gemm_names if n in stages]
     roofline = gemm_all = None
     if gemm_stages:
@@ -469,7 +498,10 @@ def run_cuda(args, cfg):
                         "peak_regime": regime, "peak_source": peaks["source"] + f", {regime} bf16"
                         + (" x 2 (assumed fp8:bf16 ratio, not measured)" if stage_peak(dom) != bf16_peak else ""),
                         "frac_tensor_burst": st["frac_measured_burst"], "frac_tensor_sustained": st["frac_measured_sustained"],
-                        "frac_tensor_nominal": st["frac_nominal"], "frac_hbm_measured": st["frac_measured_hbm"]}
+                        "frac_tensor_nominal": st["frac_nominal"], "frac_hbm_measured": st["frac_measured_hbm"],
+                        "frac_hbm_write_roof": st.get("frac_hbm_write_roof"),
+                        "write_roof_note": "bytes WRITTEN per launch / write-only bandwidth measured in this run "
+                                           "(peaks.hbm_write_gbs_measured_live); binds when above frac_hbm_measured"}
         # the aggregate the north_star's ">= 60 % of dense bf16 peak for the grouped GEMMs" is quoted on
         tsec = sum(stages[n]["ms_per_step"] for n in gemm_stages) * 1e-3
         tfl = sum(sf[n] for n in gemm_stages)
