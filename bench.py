@@ -264,30 +264,45 @@ def time_standalone_movers(moe, lb, cfg, stream, iters=20):
     Xp = torch.empty(R, H, dtype=lb.X.dtype, device="cuda")
     Y = torch.empty_like(lb.X)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    def rp():
+        moe.moe_route(lb.ccfg, z, lb.bias, idx, w, stream)
+        moe.moe_permute(lb.ccfg, lb.X, idx, counts, offsets, p2f, f2p, Xp, lb.ws, stream)
+
+    def cb():
+        moe.moe_unpermute_combine(lb.ccfg, Xp, w, f2p, None, Y, stream)
+
+    rp(); cb()
+    torch.cuda.synchronize()
+    # each call sequence is captured once and replayed, so the six small launches of route + permute are not separated
+    # by host launch gaps (the layer itself is timed the same way)
+    g_rp, g_cb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g_rp):
+        moe.moe_route(lb.ccfg, z, lb.bias, idx, w)
+        moe.moe_permute(lb.ccfg, lb.X, idx, counts, offsets, p2f, f2p, Xp, lb.ws)
+    with torch.cuda.graph(g_cb):
+        moe.moe_unpermute_combine(lb.ccfg, Xp, w, f2p, None, Y)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     t_rp, t_c = [], []
     for it in range(iters + 3):
         flush.fill_(it & 0xff)
         ev[0].record(stream)
-        moe.moe_route(lb.ccfg, z, lb.bias, idx, w, stream)
-        moe.moe_permute(lb.ccfg, lb.X, idx, counts, offsets, p2f, f2p, Xp, lb.ws, stream)
+        g_rp.replay()
         ev[1].record(stream)
         flush.fill_(it & 0xff)
         ev[2].record(stream)
-        moe.moe_unpermute_combine(lb.ccfg, Xp, w, f2p, None, Y, stream)
-        e3 = torch.cuda.Event(enable_timing=True)
-        e3.record(stream)
+        g_cb.replay()
+        ev[3].record(stream)
         torch.cuda.synchronize()
         if it >= 3:
             t_rp.append(ev[0].elapsed_time(ev[1]))
-            t_c.append(ev[2].elapsed_time(e3))
+            t_c.append(ev[2].elapsed_time(ev[3]))
     sb = stage_bytes(cfg)
     med = lambda v: sorted(v)[len(v) // 2]
     rp_bytes = sb["route"] + sb["maps"] + sb["permute"]
     return {"route_permute": {"gbs": rp_bytes / (med(t_rp) * 1e-3) / 1e9, "bytes": rp_bytes, "ms": med(t_rp),
-                              "calls": "moe_route + moe_permute, stand-alone, cold L2, median of %d" % iters},
+                              "calls": "moe_route + moe_permute, stand-alone (CUDA-graph replay), cold L2, median of %d" % iters},
             "combine": {"gbs": sb["combine"] / (med(t_c) * 1e-3) / 1e9, "bytes": sb["combine"], "ms": med(t_c),
-                        "calls": "moe_unpermute_combine, stand-alone, cold L2, median of %d" % iters}}
+                        "calls": "moe_unpermute_combine, stand-alone (CUDA-graph replay), cold L2, median of %d" % iters}}
 
 
 def run_cuda(args, cfg):

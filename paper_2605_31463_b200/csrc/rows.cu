@@ -56,14 +56,15 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
   }
 }
 
-// Zero the padding rows of every expert group: they are the tail of the group (perm_to_flat[r] < 0), at most row_align - 1
-// rows.  One CTA per expert, one warp per row, walking up from the group's end until a real row is met.
+// Zero the padding rows of every expert group: they are the tail of the group (perm_to_flat[r] < 0), at most
+// min(row_align, 128) - 1 rows.  blockIdx.x = expert, one warp per candidate row counted back from the group's end.
 __global__ void __launch_bounds__(ROW_WARPS * 32) zero_pad_kernel(const int32_t* __restrict__ p2f,
                                                                    const int32_t* __restrict__ offsets, int nvec,
                                                                    int4* __restrict__ Xp) {
   const int lane = threadIdx.x & 31;
   const int begin = offsets[blockIdx.x], end = offsets[blockIdx.x + 1];
-  for (int r = end - 1 - (int)(threadIdx.x >> 5); r >= begin && p2f[r] < 0; r -= ROW_WARPS) {
+  for (int r = end - 1 - (int)(blockIdx.y * ROW_WARPS + (threadIdx.x >> 5)); r >= begin && p2f[r] < 0;
+       r -= ROW_WARPS * gridDim.y) {
     int4* dst = Xp + (size_t)r * nvec;
     for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
   }
@@ -283,7 +284,9 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
     default: MOE_GATHER(0); break;
   }
 #undef MOE_GATHER
-  if (c->row_align > 1) MOE_LAUNCH(zero_pad_kernel, (unsigned)c->E, ROW_WARPS * 32, 0, s, p2f, offsets, nvec, (int4*)Xp);
+  if (c->row_align > 1)
+    MOE_LAUNCH(zero_pad_kernel, dim3((unsigned)c->E, (unsigned)ceil_div(std::min(c->row_align, 128), ROW_WARPS)), ROW_WARPS * 32, 0, s,
+               p2f, offsets, nvec, (int4*)Xp);
   return MOE_OK;
 }
 
@@ -343,7 +346,9 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
     }
   }
 #undef MOE_COMBINE_BWD
-  if (c->row_align > 1) MOE_LAUNCH(zero_pad_kernel, (unsigned)c->E, ROW_WARPS * 32, 0, s, p2f, offsets, nvec, (int4*)dy);
+  if (c->row_align > 1)
+    MOE_LAUNCH(zero_pad_kernel, dim3((unsigned)c->E, (unsigned)ceil_div(std::min(c->row_align, 128), ROW_WARPS)), ROW_WARPS * 32, 0, s,
+               p2f, offsets, nvec, (int4*)dy);
   return MOE_OK;
 }
 

@@ -84,7 +84,7 @@ def cmd_step(a):
             "CUDA-event stage table of the bench line, not absolutes)."]
     if a.note:
         out += ["", a.note]
-    path = os.path.join(PROFILES, f"{a.tag}_step_{a.workload}.md")
+    path = os.path.join(a.out_dir, f"{a.tag}_step_{a.workload}.md")
     open(path, "w").write("\n".join(out) + "\n")
     # traffic per launch of each GEMM stage: the routed experts' launches are the heavy ones (wgrad: three of them)
     stages = {}
@@ -92,7 +92,7 @@ def cmd_step(a):
         v = sorted(v, reverse=True)
         n = 3 if st == "wgrad" else 1
         stages[st] = sum(v[:n]) / len(v[:n])
-    tpath = os.path.join(PROFILES, "traffic.json")
+    tpath = os.path.join(a.out_dir, "traffic.json")
     try:
         rec = json.load(open(tpath))
     except (OSError, ValueError):
@@ -124,12 +124,12 @@ def cmd_launches(a):
         out.append(f"| `{k}` | {len(v)} | {sum(v) / len(v):.1f} | {100 * sum(v) / tot:.1f}% |")
     if a.note:
         out += ["", a.note]
-    path = os.path.join(PROFILES, f"{a.tag}_launches_{a.workload}.md")
+    path = os.path.join(a.out_dir, f"{a.tag}_launches_{a.workload}.md")
     open(path, "w").write("\n".join(out) + "\n")
     print(path)
 
 
-def main():
+def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     sub = ap.add_subparsers(dest="cmd", required=True)
     for name, fn in (("step", cmd_step), ("launches", cmd_launches)):
@@ -139,8 +139,9 @@ def main():
         p.add_argument("--tag", required=True)
         p.add_argument("--command", required=True)
         p.add_argument("--note", default="")
+        p.add_argument("--out-dir", default=PROFILES)
         p.set_defaults(fn=fn)
-    a = ap.parse_args()
+    a = ap.parse_args(argv)
     a.fn(a)
 
 

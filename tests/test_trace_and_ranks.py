@@ -86,3 +86,38 @@ def test_replica_timing_is_max_over_ranks_gloo():
         p.join(60)
     assert [g[1] for g in got] == [15.0, 15.0]               # every rank sees the slowest replica's time
     assert got[0][2] != got[1][2]                            # each replica draws its own batch
+
+
+def test_ncu_summary_parses_raw_and_launch_csv(tmp_path):
+    """The script that writes profiles/*.md and profiles/traffic.json (bench.py's roofline.traffic) from ncu CSV exports:
+    unit scaling, kernel naming, and the per-stage traffic (wgrad = mean of its three heaviest launches)."""
+    import json
+    from paper_2605_31463_b200 import ncu_summary
+    hdr = ["ID", "Kernel Name", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
+           "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "lts__throughput.avg.pct_of_peak_sustained_elapsed",
+           "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active", "launch__registers_per_thread", "launch__grid_size"]
+    units = ["", "", "us", "Mbyte", "Gbyte", "%", "%", "%", "register/thread", ""]
+    k = "void moe::(anonymous namespace)::tc_gemm_kernel<%d, %d, 0>(CUtensorMap_st, TcParams)"
+    rows = [[str(i), k % (m, pr), t, rd, wr, "50", "40", "60", "128", "148"] for i, (m, pr, t, rd, wr) in enumerate(
+        [(1, 0, "100", "1000", "0.5"), (4, 1, "200", "400", "0.4"), (4, 1, "210", "400", "0.4"), (4, 1, "205", "400", "0.4"),
+         (4, 1, "20", "10", "0.01")])]
+    raw = tmp_path / "raw.csv"
+    with open(raw, "w", newline="") as fh:
+        import csv
+        w = csv.writer(fh, quoting=csv.QUOTE_ALL)
+        w.writerow(hdr); w.writerow(units)
+        for r in rows:
+            w.writerow(r)
+    ncu_summary.main(["step", str(raw), "--workload", "w", "--tag", "t", "--command", "ncu ...", "--out-dir", str(tmp_path)])
+    md = (tmp_path / "t_step_w.md").read_text()
+    assert "tc_gemm_kernel<1, 0, 0> TC_FWD_SWIGLU" in md and "| 100.0 | 1000.0 | 500.0 |" in md
+    tr = json.loads((tmp_path / "traffic.json").read_text())["w"]["stages"]
+    assert abs(tr["gemm1_swiglu"] - 1.5e9) < 1 and abs(tr["wgrad"] - 0.8e9) < 1
+    lc = tmp_path / "l.csv"
+    with open(lc, "w", newline="") as fh:
+        w = csv.writer(fh, quoting=csv.QUOTE_ALL)
+        w.writerow(["ID", "Kernel Name", "Metric Name", "Metric Unit", "Metric Value"])
+        w.writerow(["0", k % (0, 0), "gpu__time_duration.sum", "ns", "2000"])
+        w.writerow(["1", k % (0, 0), "gpu__time_duration.sum", "ns", "4000"])
+    ncu_summary.main(["launches", str(lc), "--workload", "w", "--tag", "t", "--command", "ncu ...", "--out-dir", str(tmp_path)])
+    assert "| `tc_gemm_kernel<0, 0, 0> TC_FWD` | 2 | 3.0 | 100.0% |" in (tmp_path / "t_launches_w.md").read_text()
