@@ -7,6 +7,7 @@
 // dequantisation of R9 fused into the main loop, exact up to fp32 rounding of the scaled sums.  Tiles are
 // 128 rows x 128 output columns, so every tile sees exactly one weight-scale scalar per k-block (two for the
 // gate/up pair of the fused SwiGLU forward, whose tile is 64 gate + 64 up columns).
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -427,6 +428,177 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 }
 
 // ---------------------------------------------------------------------------------------------
+// the wide kernel: F8_FWD / F8_DGRAD on 128 x 256 tiles
+// ---------------------------------------------------------------------------------------------
+// The two GEMMs with a plain epilogue (y = Q(a) Q(Wd)^T and dXp = Q(dg) Q(Wg) + Q(du) Q(Wu)).  Same roles and the same
+// two-level accumulation as above, but a tile is 256 output columns wide: 48 KB of operands per 128-deep k-block feed twice
+// the MACs of a 128 x 128 tile's 32 KB (the narrow kernel is bound by that feed), the partial product
+// of a k-block lands in one of two 256-column TMEM buffers, and a promotion thread owns one row x 128 columns = exactly one
+// weight-scale column block (128 fp32 accumulators in registers).
+constexpr int WBN = 256, WSTAGES = 4, WB_BYTES = WBN * BK, WSTAGE_BYTES = A_BYTES + WB_BYTES, WNBUF = 2;
+static_assert(WSTAGES * WSTAGE_BYTES <= STAGES * STAGE_BYTES, "fits the same shared-memory allocation");
+
+__device__ __forceinline__ bool wide_tile(const F8Params& p, int64_t i, int64_t total, Tile& tl) {
+  const int64_t t = blockIdx.x + i * (int64_t)gridDim.x;
+  if (t >= total) return false;
+  const int mt = (int)(t / p.n_tiles);
+  tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * WBN;
+  tl.m0 = mt * BM;
+  tl.e = p.mtile ? p.mtile[1 + mt] : 0;
+  return true;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+f8_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
+               const __grid_constant__ CUtensorMap tmB1, const F8Params p) {
+  static_assert(MODE == F8_FWD || MODE == F8_DGRAD, "plain-epilogue modes only");
+  constexpr bool B_MN = (MODE == F8_DGRAD);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bars = base + WSTAGES * WSTAGE_BYTES;
+  const uint32_t full0 = bars, empty0 = bars + 8 * WSTAGES, pfull0 = bars + 16 * WSTAGES, pempty0 = pfull0 + 8 * WNBUF;
+  const uint32_t tmem_slot = pempty0 + 8 * WNBUF;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB0);
+    tma_prefetch_desc(&tmB1);
+    for (int s = 0; s < WSTAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 1);
+    }
+    for (int b = 0; b < WNBUF; ++b) {
+      mbar_init(pfull0 + 8 * b, 1);
+      mbar_init(pempty0 + 8 * b, EPI_WARPS);
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, WNBUF * WBN);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int64_t total = total_tiles(p);
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      Tile tl;
+      for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+        for (int kb = 0; kb < p.nkb; ++kb) {
+          mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const uint32_t fb = full0 + 8 * stage;
+          const uint32_t sa = base + stage * WSTAGE_BYTES, sb = sa + A_BYTES;
+          mbar_expect_tx(fb, WSTAGE_BYTES);
+          tma_load_2d(sa, &tmA, fb, kb * BK, tl.m0);                                   // 128 B x 128 rows
+          if (!B_MN) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);              // 128 B x 256 rows
+          } else {
+            const bool second = kb >= p.kb_split;
+            const int kr = tl.e * p.b_rows + (second ? kb - p.kb_split : kb) * BK;
+#pragma unroll
+            for (int i = 0; i < WBN / 128; ++i)                                        // 128 cols x 128 k-rows each
+              tma_load_2d(sb + i * (128 * BK), second ? &tmB1 : &tmB0, fb, tl.n0 + 128 * i, kr);
+          }
+          if (++stage == WSTAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = instr_desc(0, 0, B_MN ? 1 : 0, WBN);
+      int stage = 0, buf = 0;
+      uint32_t phase = 0, bphase = 0;
+      Tile tl;
+      for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+        for (int kb = 0; kb < p.nkb; ++kb) {
+          mbar_wait(pempty0 + 8 * buf, bphase ^ 1);
+          mbar_wait(full0 + 8 * stage, phase);
+          tc_fence_after();
+          const uint32_t sa = base + stage * WSTAGE_BYTES, sb = sa + A_BYTES;
+          const uint32_t dacc = tmem_base + buf * WBN;
+#pragma unroll
+          for (int k = 0; k < BK / UK; ++k) {
+            const uint64_t ad = smem_desc(sa + k * UK, 16, 1024);
+            // MN-major B: two 128-column boxes, 128 * BK bytes apart (LBO)
+            const uint64_t bd = B_MN ? smem_desc(sb + k * UK * 128, 128 * BK, 1024) : smem_desc(sb + k * UK, 16, 1024);
+            umma_f8(dacc, ad, bd, idesc, k != 0);
+          }
+          umma_commit(empty0 + 8 * stage);
+          umma_commit(pfull0 + 8 * buf);
+          if (++stage == WSTAGES) { stage = 0; phase ^= 1; }
+          if (++buf == WNBUF) { buf = 0; bphase ^= 1; }
+        }
+      }
+    }
+  } else {
+    // ===================== promotion + epilogue warps 2..9 =====================
+    const int lg = warp & 3;                   // TMEM lane group of this warp
+    const int ch = (warp - 2) >> 2;            // 128-column half = weight-scale column block
+    const int row_in_tile = lg * 32 + lane;
+    int buf = 0;
+    uint32_t bphase = 0;
+    Tile tl;
+    for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+      const int64_t row = (int64_t)tl.m0 + row_in_tile;
+      const bool row_ok = row < p.rows_valid;
+      const float* sa_row = p.a_scales + (row_ok ? row : 0) * p.a_nblk;
+      const int nb = tl.n0 / 128 + ch;
+      auto wscale = [&](int kb) {
+        if (!B_MN) return __ldg(p.b0_scales + ((int64_t)tl.e * (p.b_rows / 128) + nb) * p.nb_b_cols + kb);
+        const bool second = kb >= p.kb_split;
+        return __ldg((second ? p.b1_scales : p.b0_scales) +
+                     ((int64_t)tl.e * (p.b_rows / 128) + (second ? kb - p.kb_split : kb)) * p.nb_b_cols + nb);
+      };
+      float acc[128];
+#pragma unroll
+      for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+      float sa_n = __ldg(sa_row), sb_n = wscale(0);
+      for (int kb = 0; kb < p.nkb; ++kb) {
+        const float f = sa_n * sb_n;
+        if (kb + 1 < p.nkb) {
+          sa_n = __ldg(sa_row + kb + 1);
+          sb_n = wscale(kb + 1);
+        }
+        mbar_wait(pfull0 + 8 * buf, bphase);
+        tc_fence_after();
+        const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + buf * WBN + ch * 128;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          uint32_t v[32];
+          tmem_ld32(tacc + j * 32, v);
+          tmem_ld_wait();
+          if (j == 3) {                        // the buffer is drained: the MMAs of k-block kb + 2 may overwrite it
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(pempty0 + 8 * buf);
+          }
+#pragma unroll
+          for (int i = 0; i < 32; ++i) acc[j * 32 + i] = fmaf(f, __uint_as_float(v[i]), acc[j * 32 + i]);
+        }
+        if (++buf == WNBUF) { buf = 0; bphase ^= 1; }
+      }
+      if (row_ok) {
+        __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0 + ch * 128;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) *reinterpret_cast<uint4*>(dst + q * 8) = pack8(acc + q * 8);
+      }
+      __syncwarp();
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, WNBUF * WBN);
+}
+
+// ---------------------------------------------------------------------------------------------
 // host
 // ---------------------------------------------------------------------------------------------
 bool g_attr_set[MAX_DEVICES][4];   // per device
@@ -445,6 +617,31 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_tiles));
   MOE_LAUNCH(f8_gemm_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, p);
   return MOE_OK;
+}
+
+bool g_wide_attr[MAX_DEVICES][4];
+
+template <int MODE>
+int32_t launch_wide(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b1, const F8Params& p, int64_t max_tiles,
+                    cudaStream_t s) {
+  const int dev = current_device();
+  if (dev < 0) return MOE_ERR_CUDA;
+  if (!g_wide_attr[dev][MODE]) {
+    MOE_CUDA(cudaFuncSetAttribute(f8_wide_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    g_wide_attr[dev][MODE] = true;
+  }
+  const int sms = tc_sm_count();
+  if (sms <= 0) return MOE_ERR_CUDA;
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, max_tiles));
+  MOE_LAUNCH(f8_wide_kernel<MODE>, grid, NTHREADS, SMEM_BYTES, s, a, b0, b1, p);
+  return MOE_OK;
+}
+
+// 128 x 256 tiles for the plain-epilogue GEMMs when the output width allows; MOE_B200_FP8_WIDE=0 (debug knob) keeps 128 x 128
+bool use_wide(int N) {
+  const char* e = getenv("MOE_B200_FP8_WIDE");
+  if (e && e[0] == '0') return false;
+  return N % WBN == 0;
 }
 
 }  // namespace
@@ -485,9 +682,11 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
     case F8_FWD: {
       if (c.lda != c.b_cols || c.N != c.b_rows) return MOE_ERR_INVALID_ARG;
       p.nkb = c.b_cols / BK;
-      p.n_tiles = c.N / BN;
+      const bool wide = use_wide(c.N);
+      p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
-      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, BN)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, wide ? WBN : BN)) return MOE_ERR_UNSUPPORTED;
+      if (wide) return launch_wide<F8_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
       return launch<F8_FWD>(ta, tb0, tb0, p, max_mtiles * p.n_tiles, s);
     }
     case F8_FWD_SWIGLU: {
@@ -505,10 +704,12 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
       if (c.N != c.b_cols || c.lda != (split ? 2 : 1) * c.b_rows) return MOE_ERR_INVALID_ARG;
       p.kb_split = c.b_rows / BK;
       p.nkb = split ? 2 * p.kb_split : p.kb_split;
-      p.n_tiles = c.N / BN;
+      const bool wide = c.mode == F8_DGRAD && use_wide(c.N);
+      p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb1, 1, split ? c.B1 : c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
+      if (wide) return launch_wide<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
       if (c.mode == F8_DGRAD) return launch<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
       if (!c.gu || c.F != c.b_cols || (c.ldgu & 7)) return MOE_ERR_INVALID_ARG;
       return launch<F8_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
