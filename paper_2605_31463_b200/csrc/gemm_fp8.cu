@@ -430,19 +430,20 @@ f8_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // ---------------------------------------------------------------------------------------------
 // the wide kernel: F8_FWD / F8_DGRAD on 128 x 256 tiles
 // ---------------------------------------------------------------------------------------------
-// The two GEMMs with a plain epilogue (y = Q(a) Q(Wd)^T and dXp = Q(dg) Q(Wg) + Q(du) Q(Wu)).  Same roles and the same
-// two-level accumulation as above, but a tile is 256 output columns wide: 48 KB of operands per 128-deep k-block feed twice
+// All four modes when the output width allows.  Same roles and the same two-level accumulation as above, but a tile is
+// 256 accumulator columns wide (the fused SwiGLU forward: 128 gate + 128 up columns = one whole 1 x 128 block of a): 48 KB of operands per 128-deep k-block feed twice
 // the MACs of a 128 x 128 tile's 32 KB (the narrow kernel is bound by that feed), the partial product
 // of a k-block lands in one of two 256-column TMEM buffers, and a promotion thread owns one row x 128 columns = exactly one
 // weight-scale column block (128 fp32 accumulators in registers).
 constexpr int WBN = 256, WSTAGES = 4, WB_BYTES = WBN * BK, WSTAGE_BYTES = A_BYTES + WB_BYTES, WNBUF = 2;
 static_assert(WSTAGES * WSTAGE_BYTES <= STAGES * STAGE_BYTES, "fits the same shared-memory allocation");
 
+template <int MODE>
 __device__ __forceinline__ bool wide_tile(const F8Params& p, int64_t i, int64_t total, Tile& tl) {
   const int64_t t = blockIdx.x + i * (int64_t)gridDim.x;
   if (t >= total) return false;
   const int mt = (int)(t / p.n_tiles);
-  tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * WBN;
+  tl.n0 = (int)(t - (int64_t)mt * p.n_tiles) * (MODE == F8_FWD_SWIGLU ? WBN / 2 : WBN);   // SwiGLU: 128 gate + 128 up
   tl.m0 = mt * BM;
   tl.e = p.mtile ? p.mtile[1 + mt] : 0;
   return true;
@@ -452,11 +453,11 @@ template <int MODE>
 __global__ void __launch_bounds__(NTHREADS, 1)
 f8_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
                const __grid_constant__ CUtensorMap tmB1, const F8Params p) {
-  static_assert(MODE == F8_FWD || MODE == F8_DGRAD, "plain-epilogue modes only");
-  constexpr bool B_MN = (MODE == F8_DGRAD);
+  constexpr bool B_MN = (MODE == F8_DGRAD || MODE == F8_DGRAD_SWIGLU);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bars = base + WSTAGES * WSTAGE_BYTES;
+  float* const xch = reinterpret_cast<float*>(smem_raw + (base - smem_u32(smem_raw)) + WSTAGES * WSTAGE_BYTES);
+  const uint32_t bars = base + WSTAGES * WSTAGE_BYTES + XCH_BYTES;
   const uint32_t full0 = bars, empty0 = bars + 8 * WSTAGES, pfull0 = bars + 16 * WSTAGES, pempty0 = pfull0 + 8 * WNBUF;
   const uint32_t tmem_slot = pempty0 + 8 * WNBUF;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -490,15 +491,18 @@ f8_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       int stage = 0;
       uint32_t phase = 0;
       Tile tl;
-      for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+      for (int64_t t = 0; wide_tile<MODE>(p, t, total, tl); ++t) {
         for (int kb = 0; kb < p.nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, phase ^ 1);
           const uint32_t fb = full0 + 8 * stage;
           const uint32_t sa = base + stage * WSTAGE_BYTES, sb = sa + A_BYTES;
           mbar_expect_tx(fb, WSTAGE_BYTES);
           tma_load_2d(sa, &tmA, fb, kb * BK, tl.m0);                                   // 128 B x 128 rows
-          if (!B_MN) {
+          if (MODE == F8_FWD) {
             tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);              // 128 B x 256 rows
+          } else if (MODE == F8_FWD_SWIGLU) {
+            tma_load_2d(sb, &tmB0, fb, kb * BK, tl.e * p.b_rows + tl.n0);              // 128 B x 128 rows (Wg)
+            tma_load_2d(sb + WB_BYTES / 2, &tmB1, fb, kb * BK, tl.e * p.b_rows + tl.n0);   // (Wu)
           } else {
             const bool second = kb >= p.kb_split;
             const int kr = tl.e * p.b_rows + (second ? kb - p.kb_split : kb) * BK;
@@ -517,7 +521,7 @@ f8_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       int stage = 0, buf = 0;
       uint32_t phase = 0, bphase = 0;
       Tile tl;
-      for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+      for (int64_t t = 0; wide_tile<MODE>(p, t, total, tl); ++t) {
         for (int kb = 0; kb < p.nkb; ++kb) {
           mbar_wait(pempty0 + 8 * buf, bphase ^ 1);
           mbar_wait(full0 + 8 * stage, phase);
@@ -540,55 +544,191 @@ f8_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
   } else {
     // ===================== promotion + epilogue warps 2..9 =====================
+    // A thread owns one row and 128 accumulator columns: columns [ch * 128, + 128) of the tile, or for the fused SwiGLU
+    // forward 64 gate columns [ch * 64, + 64) and the 64 up columns of the same outputs [128 + ch * 64, + 64).
+    constexpr bool SW = (MODE == F8_FWD_SWIGLU);
     const int lg = warp & 3;                   // TMEM lane group of this warp
-    const int ch = (warp - 2) >> 2;            // 128-column half = weight-scale column block
+    const int ch = (warp - 2) >> 2;
     const int row_in_tile = lg * 32 + lane;
+    const int c0 = SW ? ch * 64 : ch * 128;                 // first TMEM column of accumulators 0..63
+    const int c1 = SW ? 128 + ch * 64 : ch * 128 + 64;      // ... and of accumulators 64..127
     int buf = 0;
     uint32_t bphase = 0;
     Tile tl;
-    for (int64_t t = 0; wide_tile(p, t, total, tl); ++t) {
+    for (int64_t t = 0; wide_tile<MODE>(p, t, total, tl); ++t) {
       const int64_t row = (int64_t)tl.m0 + row_in_tile;
       const bool row_ok = row < p.rows_valid;
       const float* sa_row = p.a_scales + (row_ok ? row : 0) * p.a_nblk;
-      const int nb = tl.n0 / 128 + ch;
-      auto wscale = [&](int kb) {
-        if (!B_MN) return __ldg(p.b0_scales + ((int64_t)tl.e * (p.b_rows / 128) + nb) * p.nb_b_cols + kb);
-        const bool second = kb >= p.kb_split;
-        return __ldg((second ? p.b1_scales : p.b0_scales) +
-                     ((int64_t)tl.e * (p.b_rows / 128) + (second ? kb - p.kb_split : kb)) * p.nb_b_cols + nb);
+      const int nb = tl.n0 / 128 + (SW ? 0 : ch);             // weight-scale column block of this thread
+      // weight scale(s) of k-block kb: one scalar, or the gate / up pair of the SwiGLU forward
+      auto wscale = [&](int kb, float& s0, float& s1) {
+        if (MODE == F8_FWD || SW) {
+          const int64_t i = ((int64_t)tl.e * (p.b_rows / 128) + nb) * p.nb_b_cols + kb;
+          s0 = __ldg(p.b0_scales + i);
+          s1 = SW ? __ldg(p.b1_scales + i) : s0;
+        } else {
+          const bool second = kb >= p.kb_split;
+          s0 = s1 = __ldg((second ? p.b1_scales : p.b0_scales) +
+                          ((int64_t)tl.e * (p.b_rows / 128) + (second ? kb - p.kb_split : kb)) * p.nb_b_cols + nb);
+        }
       };
       float acc[128];
 #pragma unroll
       for (int i = 0; i < 128; ++i) acc[i] = 0.f;
-      float sa_n = __ldg(sa_row), sb_n = wscale(0);
+      float sa_n = __ldg(sa_row), s0_n, s1_n;
+      wscale(0, s0_n, s1_n);
       for (int kb = 0; kb < p.nkb; ++kb) {
-        const float f = sa_n * sb_n;
+        const float f0 = sa_n * s0_n, f1 = sa_n * s1_n;
         if (kb + 1 < p.nkb) {
           sa_n = __ldg(sa_row + kb + 1);
-          sb_n = wscale(kb + 1);
+          wscale(kb + 1, s0_n, s1_n);
         }
         mbar_wait(pfull0 + 8 * buf, bphase);
         tc_fence_after();
-        const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + buf * WBN + ch * 128;
+        const uint32_t tacc = tmem_base + ((uint32_t)(lg * 32) << 16) + buf * WBN;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           uint32_t v[32];
-          tmem_ld32(tacc + j * 32, v);
+          tmem_ld32(tacc + (j < 2 ? c0 + j * 32 : c1 + (j - 2) * 32), v);
           tmem_ld_wait();
           if (j == 3) {                        // the buffer is drained: the MMAs of k-block kb + 2 may overwrite it
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(pempty0 + 8 * buf);
           }
+          const float f = j < 2 ? f0 : f1;
 #pragma unroll
           for (int i = 0; i < 32; ++i) acc[j * 32 + i] = fmaf(f, __uint_as_float(v[i]), acc[j * 32 + i]);
         }
         if (++buf == WNBUF) { buf = 0; bphase ^= 1; }
       }
-      if (row_ok) {
-        __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0 + ch * 128;
+      if (MODE == F8_FWD || MODE == F8_DGRAD) {
+        if (row_ok) {
+          __nv_bfloat16* dst = p.out0 + row * p.ld0 + tl.n0 + ch * 128;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) *reinterpret_cast<uint4*>(dst + q * 8) = pack8(acc + q * 8);
+          for (int q = 0; q < 16; ++q) *reinterpret_cast<uint4*>(dst + q * 8) = pack8(acc + q * 8);
+        }
+      } else if (SW) {
+        // g = acc[0..63], u = acc[64..127] of output columns n0 + ch * 64 ..; a = silu(g) * u
+        const int col = tl.n0 + ch * 64;
+        __nv_bfloat16* gdst = p.out0 + row * p.ld0 + col;
+        __nv_bfloat16* adst = p.out1 + row * p.ld1 + col;
+        if (row_ok) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            *reinterpret_cast<uint4*>(gdst + q * 8) = pack8(acc + q * 8);
+            *reinterpret_cast<uint4*>(gdst + p.F + q * 8) = pack8(acc + 64 + q * 8);
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < 64; ++i) acc[i] = acc[i] * fast_sigmoid8(acc[i]) * acc[64 + i];
+        uint4 ab[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          ab[q] = pack8(acc + q * 8);
+          if (row_ok) *reinterpret_cast<uint4*>(adst + q * 8) = ab[q];
+        }
+        if (p.q_codes) {
+          // fused Q-a (R9): quantise the bf16 a just written, 1 x 128 along F = this tile's 128 columns, shared with the
+          // other column-half warp of the lane group (amax exchanged through shared memory, double-buffered by tile parity)
+          float am = 0.f;
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const uint32_t wv[4] = {ab[q].x, ab[q].y, ab[q].z, ab[q].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) am = fmaxf(am, fmaxf(fabsf(bf16_lo(wv[i])), fabsf(bf16_hi(wv[i]))));
+          }
+          float* slot = xch + ((t & 1) * BM + row_in_tile) * 2;
+          slot[ch] = am;
+          named_bar_sync(1 + lg, 64);
+          const float sc = fp8_block_scale(fmaxf(slot[0], slot[1]), p.q_mode);
+          const float isc = 1.0f / sc;
+          if (row_ok) {
+            uint8_t* cdst = p.q_codes + row * (int64_t)p.F + col;
+#pragma unroll
+            for (int q = 0; q < 8; q += 2) {
+              uint32_t e[4];
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const uint4 va = ab[q + h];
+                e[2 * h] = enc4(bf16_lo(va.x), bf16_hi(va.x), bf16_lo(va.y), bf16_hi(va.y), sc, isc, p.q_mode);
+                e[2 * h + 1] = enc4(bf16_lo(va.z), bf16_hi(va.z), bf16_lo(va.w), bf16_hi(va.w), sc, isc, p.q_mode);
+              }
+              *reinterpret_cast<uint4*>(cdst + q * 8) = make_uint4(e[0], e[1], e[2], e[3]);
+            }
+            if (ch == 0) p.q_scales[row * (int64_t)(p.F / 128) + tl.n0 / 128] = sc;
+          }
+        }
+      } else {
+        // F8_DGRAD_SWIGLU: acc = da of columns [n0 + ch * 128, + 128) of F: one whole 1 x 128 block of dg and one of du
+        float rw = 1.0f;
+        if (p.w && row_ok) {
+          const int pf = p.p2f[row];
+          rw = pf >= 0 ? p.w[pf] : 0.f;
+        }
+        const int col = tl.n0 + ch * 128;
+        const __nv_bfloat16* gsrc = p.gu + row * p.ldgu + col;
+        __nv_bfloat16* dgdst = p.out0 + row * p.ld0 + col;
+        float amg = 0.f, amu = 0.f;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          uint4 gq = make_uint4(0u, 0u, 0u, 0u), uq = gq;
+          if (row_ok) {
+            gq = *reinterpret_cast<const uint4*>(gsrc + q * 8);
+            uq = *reinterpret_cast<const uint4*>(gsrc + p.F + q * 8);
+          }
+          const uint32_t gw[4] = {gq.x, gq.y, gq.z, gq.w}, uw[4] = {uq.x, uq.y, uq.z, uq.w};
+          float og[8], ou[8];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float g0 = bf16_lo(gw[i]), g1 = bf16_hi(gw[i]), u0 = bf16_lo(uw[i]), u1 = bf16_hi(uw[i]);
+            const float d0 = rw * acc[q * 8 + 2 * i], d1 = rw * acc[q * 8 + 2 * i + 1];
+            const float s0 = fast_sigmoid8(g0), s1 = fast_sigmoid8(g1);
+            og[2 * i] = d0 * u0 * s0 * (1.0f + g0 * (1.0f - s0));
+            og[2 * i + 1] = d1 * u1 * s1 * (1.0f + g1 * (1.0f - s1));
+            ou[2 * i] = d0 * g0 * s0;
+            ou[2 * i + 1] = d1 * g1 * s1;
+          }
+          const uint4 pg = pack8(og), pu = pack8(ou);
+          if (row_ok) {
+            *reinterpret_cast<uint4*>(dgdst + q * 8) = pg;
+            *reinterpret_cast<uint4*>(dgdst + p.F + q * 8) = pu;
+          }
+          const uint32_t wg[4] = {pg.x, pg.y, pg.z, pg.w}, wu[4] = {pu.x, pu.y, pu.z, pu.w};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            amg = fmaxf(amg, fmaxf(fabsf(bf16_lo(wg[i])), fabsf(bf16_hi(wg[i]))));
+            amu = fmaxf(amu, fmaxf(fabsf(bf16_lo(wu[i])), fabsf(bf16_hi(wu[i]))));
+          }
+        }
+        if (p.q_codes && row_ok) {
+          // fused Q-dgu (R9): the thread holds the amax of its whole dg block and du block; the bf16 values are its own
+          // stores of a moment ago, read back (L2-hot, same thread: program order) instead of 128 more live registers
+          const float sg = fp8_block_scale(amg, p.q_mode), su = fp8_block_scale(amu, p.q_mode);
+          const float isg = 1.0f / sg, isu = 1.0f / su;
+          uint8_t* cg = p.q_codes + row * (int64_t)(2 * p.F) + col;
+          const volatile uint4* rg = reinterpret_cast<const volatile uint4*>(dgdst);
+          const volatile uint4* ru = reinterpret_cast<const volatile uint4*>(dgdst + p.F);
+#pragma unroll
+          for (int q = 0; q < 16; q += 2) {
+            uint32_t eg[4], eu[4];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              uint4 vg, vu;
+              vg.x = rg[q + h].x; vg.y = rg[q + h].y; vg.z = rg[q + h].z; vg.w = rg[q + h].w;
+              vu.x = ru[q + h].x; vu.y = ru[q + h].y; vu.z = ru[q + h].z; vu.w = ru[q + h].w;
+              eg[2 * h] = enc4(bf16_lo(vg.x), bf16_hi(vg.x), bf16_lo(vg.y), bf16_hi(vg.y), sg, isg, p.q_mode);
+              eg[2 * h + 1] = enc4(bf16_lo(vg.z), bf16_hi(vg.z), bf16_lo(vg.w), bf16_hi(vg.w), sg, isg, p.q_mode);
+              eu[2 * h] = enc4(bf16_lo(vu.x), bf16_hi(vu.x), bf16_lo(vu.y), bf16_hi(vu.y), su, isu, p.q_mode);
+              eu[2 * h + 1] = enc4(bf16_lo(vu.z), bf16_hi(vu.z), bf16_lo(vu.w), bf16_hi(vu.w), su, isu, p.q_mode);
+            }
+            *reinterpret_cast<uint4*>(cg + q * 8) = make_uint4(eg[0], eg[1], eg[2], eg[3]);
+            *reinterpret_cast<uint4*>(cg + p.F + q * 8) = make_uint4(eu[0], eu[1], eu[2], eu[3]);
+          }
+          float* sc = p.q_scales + row * (int64_t)(2 * p.F / 128);
+          sc[col / 128] = sg;
+          sc[(p.F + col) / 128] = su;
+        }
       }
       __syncwarp();
     }
@@ -637,11 +777,14 @@ int32_t launch_wide(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorM
   return MOE_OK;
 }
 
-// 128 x 256 tiles for the plain-epilogue GEMMs when the output width allows; MOE_B200_FP8_WIDE=0 (debug knob) keeps 128 x 128
-bool use_wide(int N) {
+// 128 x 256 tiles when the output width allows.  Default (1): the plain-epilogue GEMMs (gemm2, dgrad gate/up: configs[3]
+// 1.46 -> 1.16 ms, 2.71 -> 2.51 ms).  The fused-SwiGLU modes run on the wide kernel too (parity-tested) but slower (gemm1
+// 2.66 -> 2.86 ms, dgrad-down 1.67 -> 1.78 ms): their long epilogues are not overlapped with the next tile's main loop, and
+// two TMEM buffers give the MMAs less slack than four.  MOE_B200_FP8_WIDE = 0 (never) / 1 / 2 (all modes); debug knob.
+bool use_wide(int N, bool swiglu) {
   const char* e = getenv("MOE_B200_FP8_WIDE");
-  if (e && e[0] == '0') return false;
-  return N % WBN == 0;
+  const int level = (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
+  return level > (swiglu ? 1 : 0) && N % WBN == 0;
 }
 
 }  // namespace
@@ -682,7 +825,7 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
     case F8_FWD: {
       if (c.lda != c.b_cols || c.N != c.b_rows) return MOE_ERR_INVALID_ARG;
       p.nkb = c.b_cols / BK;
-      const bool wide = use_wide(c.N);
+      const bool wide = use_wide(c.N, false);
       p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, wide ? WBN : BN)) return MOE_ERR_UNSUPPORTED;
@@ -692,10 +835,12 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
     case F8_FWD_SWIGLU: {
       if (!c.B1 || !c.b1_scales || !c.out1 || c.lda != c.b_cols || c.F != c.b_rows || (c.ld1 & 7)) return MOE_ERR_INVALID_ARG;
       p.nkb = c.b_cols / BK;
-      p.n_tiles = c.F / (BN / 2);
+      const bool wide = use_wide(2 * c.F, true);          // a wide tile = 128 gate + 128 up columns: F is a multiple of 128 already
+      p.n_tiles = c.F / ((wide ? WBN : BN) / 2);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
-      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, BN / 2)) return MOE_ERR_UNSUPPORTED;
-      if (!tc_make_map(&tb1, 1, c.B1, c.b_cols, wrows, c.b_cols, BK, BN / 2)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, (wide ? WBN : BN) / 2)) return MOE_ERR_UNSUPPORTED;
+      if (!tc_make_map(&tb1, 1, c.B1, c.b_cols, wrows, c.b_cols, BK, (wide ? WBN : BN) / 2)) return MOE_ERR_UNSUPPORTED;
+      if (wide) return launch_wide<F8_FWD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
       return launch<F8_FWD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
     }
     case F8_DGRAD:
@@ -704,14 +849,17 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
       if (c.N != c.b_cols || c.lda != (split ? 2 : 1) * c.b_rows) return MOE_ERR_INVALID_ARG;
       p.kb_split = c.b_rows / BK;
       p.nkb = split ? 2 * p.kb_split : p.kb_split;
-      const bool wide = c.mode == F8_DGRAD && use_wide(c.N);
+      const bool wide = use_wide(c.N, c.mode == F8_DGRAD_SWIGLU);
       p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb1, 1, split ? c.B1 : c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;
-      if (wide) return launch_wide<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
-      if (c.mode == F8_DGRAD) return launch<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      if (c.mode == F8_DGRAD) {
+        if (wide) return launch_wide<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+        return launch<F8_DGRAD>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
+      }
       if (!c.gu || c.F != c.b_cols || (c.ldgu & 7)) return MOE_ERR_INVALID_ARG;
+      if (wide) return launch_wide<F8_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
       return launch<F8_DGRAD_SWIGLU>(ta, tb0, tb1, p, max_mtiles * p.n_tiles, s);
     }
   }

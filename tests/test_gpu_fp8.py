@@ -150,6 +150,28 @@ def test_fused_epilogue_quantisers_are_bit_exact(env, mode, fused, monkeypatch):
     assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq_s"))[:R], sc)
 
 
+@pytest.mark.parametrize("wide", ["0", "2"])
+def test_fp8_tile_width_levels(env, wide, monkeypatch):
+    """The FP8 GEMMs run 128 x 256 tiles for the plain-epilogue modes by default (MOE_B200_FP8_WIDE=1; the other tests).
+    =0 keeps every GEMM on 128 x 128 tiles, =2 puts the fused-SwiGLU modes on the wide kernel too: same oracle, same
+    tolerance, and the fused quantisers' codes and scales stay bit-exact."""
+    torch, moe, buffers = env
+    monkeypatch.setenv("MOE_B200_FP8_WIDE", wide)
+    monkeypatch.setenv("MOE_B200_FP8_FUSED_QUANT", "1")
+    for mode in (0, 1):
+        cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode)
+        inp = gc.gen_inputs(cfg)
+        lb = gc.run_gpu_layer(cfg, inp)
+        gc.compare_layer(cfg, inp, lb)
+        R = int(buffers.to_numpy(lb.ctx_view("offsets"))[-1])
+        codes, sc = orc.quantize_1x128(buffers.to_numpy(lb.ctx_view("a"))[:R], mode)
+        assert np.array_equal(buffers.to_numpy(lb.ctx_view("aq"))[:R], codes)
+        assert np.array_equal(buffers.to_numpy(lb.ctx_view("aq_s"))[:R], sc)
+        codes, sc = orc.quantize_1x128(buffers.to_numpy(lb.ws_view("dgu"))[:R], mode)
+        assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq"))[:R], codes)
+        assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq_s"))[:R], sc)
+
+
 def test_fp8_weight_cache_matches_oracle(env):
     """FP8 weight cache: quantise the weights once with moe_fp8_quantize_weights, then run a NEW
     micro-batch through moe_layer_fwd with NULL weights (the bf16 weights overwritten with garbage first, so nothing
