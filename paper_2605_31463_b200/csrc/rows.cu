@@ -106,8 +106,10 @@ struct Vec<__nv_bfloat16> {
 
 // Y[t] = sum_j w[t,j] * y[f2p[t*K+j]]  (+ add0[t]) (+ add1[t])  (+ sum_j dz[t,j] * Wr[idx[t,j]]);  w == NULL -> 1.
 // Empty slots (f2p = -1, variable-k routing) contribute nothing.
+// K = 8: capped at 40 registers so that 6 CTAs (48 warps) are resident per SM -- the kernel waits on its row loads, and more
+// warps in flight moved configs[1] from 71 to 50 us and configs[2] from 135 to 104 us (K = 4 was slower that way).
 template <typename T, int KT, bool SLABBED>
-__global__ void __launch_bounds__(ROW_WARPS * 32) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
+__global__ void __launch_bounds__(ROW_WARPS * 32, KT == 8 ? 6 : 1) combine_kernel(const int4* __restrict__ y, const float* __restrict__ w,
                                                                   const int32_t* __restrict__ f2p,
                                                                   const int4* __restrict__ add0,
                                                                   const int4* __restrict__ add1,
