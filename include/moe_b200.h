@@ -273,10 +273,12 @@ int32_t moe_layer_step_host_pipelined(void* pipeline, const moe_config_t* cfg, i
  * name in {"z","counts","offsets","perm_to_flat","flat_to_perm","Xp","gu","a","y","gu_s","a_s","y_s",
  *          "aux_f","aux_P","aux_loss" (fp32 [E], [E], [1]; aux_coef != 0),
  *          "aq","aq_s" (dtype 2: e4m3 codes [TK_pad,F] and fp32 scales [TK_pad,F/128] of a, written by the GEMM-1 epilogue)}.
+ * With moe_layer_rows_fused(cfg) >= 1 "a" and "y" carry the row's routing weight (w_r a_r, w_r y_r).
  * Writes the byte offset inside ctx and the byte length.  */
 int32_t moe_ctx_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
 /* Same for ws after moe_layer_bwd: {"dw","dz","dy","dgu","dXp","dz_dense" (fp32 [T,E]; dense router backward only),
- * "dguq","dguq_s" (dtype 2: codes [TK_pad,2F] / scales [TK_pad,2F/128] of [dg|du], written by the dgrad-down epilogue)}. */
+ * "dguq","dguq_s" (dtype 2: codes [TK_pad,2F] / scales [TK_pad,2F/128] of [dg|du], written by the dgrad-down epilogue)}.
+ * "dy" is w_r dY[t_r] with moe_layer_rows_fused(cfg) == 0 and the unweighted row dY[t_r] otherwise. */
 int32_t moe_ws_field(const moe_config_t* cfg, const char* name, size_t* byte_offset, size_t* byte_len);
 
 /* Stage timing for bench.py: while enabled, moe_layer_fwd / moe_layer_bwd record a CUDA event on
