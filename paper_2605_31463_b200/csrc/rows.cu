@@ -24,19 +24,40 @@ __device__ __forceinline__ void stg_stream(int4* p, const int4& v) {
                "r"(v.w));
 }
 
-// Xp[f2p[t*K+j]] = X[t] for j < K: token-major, the source row is read once and written K times.
+// Xp[f2p[t*K+j]] = X[t] for j < K: token-major, the source row is read once and written K times.  The CTAs past the token
+// range zero the padding rows of the expert groups instead (pad_blocks = E x PAD_CTAS of them; see zero_pad_rows).
+constexpr int PAD_CTAS = 16;       // x ROW_WARPS warps = 128 candidate rows per expert and pass
+__device__ __forceinline__ void zero_pad_rows(const int32_t* __restrict__ p2f, const int32_t* __restrict__ offsets, int e, int sub,
+                                              int v0, int v1, int nvec, int4* __restrict__ Xp) {
+  // the padding rows are the tail of the group (perm_to_flat[r] < 0): one warp per candidate row counted back from its end
+  const int lane = threadIdx.x & 31;
+  const int begin = offsets[e], end = offsets[e + 1];
+  for (int r = end - 1 - (sub * ROW_WARPS + (int)(threadIdx.x >> 5)); r >= begin && p2f[r] < 0; r -= ROW_WARPS * PAD_CTAS) {
+    int4* dst = Xp + (size_t)r * nvec;
+    for (int v = v0 + lane; v < v1; v += 32) dst[v] = make_int4(0, 0, 0, 0);
+  }
+}
+
 template <int KT>
 __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __restrict__ X, int T, int Krt, int nvec,
                                                                  const int32_t* __restrict__ f2p,
+                                                                 const int32_t* __restrict__ p2f,
+                                                                 const int32_t* __restrict__ offsets, int tok_blocks,
                                                                  int4* __restrict__ Xp) {
   const int K = KT > 0 ? KT : Krt;
   const int lane = threadIdx.x & 31;
+  // blockIdx.y = 2 KB column slab of the row: enough CTAs for several waves even when T / 8 is about one wave
+  const int v_lo = blockIdx.y * 128, v_hi = min(nvec, (int)(blockIdx.y + 1) * 128);
+  if ((int)blockIdx.x >= tok_blocks) {
+    const int pb = blockIdx.x - tok_blocks;
+    zero_pad_rows(p2f, offsets, pb / PAD_CTAS, pb % PAD_CTAS, v_lo, v_hi, nvec, Xp);
+    return;
+  }
   const int t = blockIdx.x * ROW_WARPS + (threadIdx.x >> 5);
   if (t >= T) return;
   const int4* src = X + (size_t)t * nvec;
   const int32_t* rows = f2p + (size_t)t * K;
-  // blockIdx.y = 2 KB column slab of the row: enough CTAs for several waves even when T / 8 is about one wave
-  for (int v0 = blockIdx.y * 128; v0 < min(nvec, (int)(blockIdx.y + 1) * 128); v0 += 128) {
+  for (int v0 = v_lo; v0 < v_hi; v0 += 128) {
     int4 buf[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -56,18 +77,11 @@ __global__ void __launch_bounds__(ROW_WARPS * 32) gather_kernel(const int4* __re
   }
 }
 
-// Zero the padding rows of every expert group: they are the tail of the group (perm_to_flat[r] < 0), at most
-// min(row_align, 128) - 1 rows.  blockIdx.x = expert, one warp per candidate row counted back from the group's end.
+// The same padding-row zeroing as a kernel of its own (after combine-backward): blockIdx = (expert, sub-range).
 __global__ void __launch_bounds__(ROW_WARPS * 32) zero_pad_kernel(const int32_t* __restrict__ p2f,
                                                                    const int32_t* __restrict__ offsets, int nvec,
                                                                    int4* __restrict__ Xp) {
-  const int lane = threadIdx.x & 31;
-  const int begin = offsets[blockIdx.x], end = offsets[blockIdx.x + 1];
-  for (int r = end - 1 - (int)(blockIdx.y * ROW_WARPS + (threadIdx.x >> 5)); r >= begin && p2f[r] < 0;
-       r -= ROW_WARPS * gridDim.y) {
-    int4* dst = Xp + (size_t)r * nvec;
-    for (int v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
-  }
+  zero_pad_rows(p2f, offsets, blockIdx.x, blockIdx.y, 0, nvec, nvec, Xp);
 }
 
 template <typename T>
@@ -276,9 +290,11 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
                     const int32_t* offsets, void* Xp, cudaStream_t s) {
   if ((cols * esz) % 16 != 0) return MOE_ERR_UNSUPPORTED;
   const int nvec = (int)(cols * esz / 16);
+  const int tok_blocks = (int)ceil_div(c->T, ROW_WARPS);
+  const int pad_blocks = c->row_align > 1 ? c->E * PAD_CTAS : 0;      // padding rows exist only with aligned groups
 #define MOE_GATHER(KT)                                                                                              \
-  MOE_LAUNCH(gather_kernel<KT>, dim3((unsigned)ceil_div(c->T, ROW_WARPS), (unsigned)ceil_div(nvec, 128)), ROW_WARPS * 32, 0, s, \
-             (const int4*)X, c->T, c->K, nvec, f2p, (int4*)Xp)
+  MOE_LAUNCH(gather_kernel<KT>, dim3((unsigned)(tok_blocks + pad_blocks), (unsigned)ceil_div(nvec, 128)), ROW_WARPS * 32, 0, s, \
+             (const int4*)X, c->T, c->K, nvec, f2p, p2f, offsets, tok_blocks, (int4*)Xp)
   switch (c->K) {
     case 2: MOE_GATHER(2); break;
     case 4: MOE_GATHER(4); break;
@@ -286,9 +302,6 @@ int32_t gather_rows(const moe_config_t* c, const void* X, int cols, size_t esz, 
     default: MOE_GATHER(0); break;
   }
 #undef MOE_GATHER
-  if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, dim3((unsigned)c->E, (unsigned)ceil_div(std::min(c->row_align, 128), ROW_WARPS)), ROW_WARPS * 32, 0, s,
-               p2f, offsets, nvec, (int4*)Xp);
   return MOE_OK;
 }
 
@@ -349,8 +362,7 @@ int32_t combine_bwd(const moe_config_t* c, const void* dY, const void* y, const 
   }
 #undef MOE_COMBINE_BWD
   if (c->row_align > 1)
-    MOE_LAUNCH(zero_pad_kernel, dim3((unsigned)c->E, (unsigned)ceil_div(std::min(c->row_align, 128), ROW_WARPS)), ROW_WARPS * 32, 0, s,
-               p2f, offsets, nvec, (int4*)dy);
+    MOE_LAUNCH(zero_pad_kernel, dim3((unsigned)c->E, PAD_CTAS), ROW_WARPS * 32, 0, s, p2f, offsets, nvec, (int4*)dy);
   return MOE_OK;
 }
 
