@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(256) dwr_tile_kernel(const float* __restrict__
                                                        const int32_t* __restrict__ mtile,
                                                        const int32_t* __restrict__ offsets,
                                                        const int32_t* __restrict__ counts, int H,
-                                                       const int32_t* __restrict__ p2f, int K,
+                                                       const int32_t* __restrict__ p2f, int K, int kshift,
                                                        float* __restrict__ part) {
   // p2f != nullptr: Xp is the TOKEN-major X [T,H] and permuted row r reads token row p2f[r] / K -- X (T H bytes) stays in
   // L2 across the K experts that touch each row, the row-grouped copy (K times larger) would stream from HBM
@@ -153,7 +153,8 @@ __global__ void __launch_bounds__(256) dwr_tile_kernel(const float* __restrict__
       const int r = r0 + i;
       if (r >= live_end) break;
       const float d = dzp[r];
-      const size_t src = p2f ? (size_t)(p2f[r] / K) : (size_t)r;          // live rows only: p2f[r] >= 0
+      // live rows only: p2f[r] >= 0; kshift >= 0: K = 2^kshift (no integer division per row and thread)
+      const size_t src = p2f ? (size_t)(kshift >= 0 ? p2f[r] >> kshift : p2f[r] / K) : (size_t)r;
       const uint4 v = __ldg(Xp + (src * H + col) / 8);
       const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
@@ -485,8 +486,11 @@ int32_t router_bwd(const moe_config_t* c, const float* z, const int32_t* idx, co
   if (dWr && c->dtype != 0 && c->row_align % 128 == 0 && c->H % 8 == 0 && mtile && part) {
     const unsigned slabs = (unsigned)ceil_div(c->H, 256);
     const bool tok = X != nullptr && p2f != nullptr;     // read the token-major X through the map
+    int kshift = -1;
+    for (int sh = 0; sh < 31; ++sh)
+      if ((1 << sh) == c->K) kshift = sh;
     MOE_LAUNCH(dwr_tile_kernel, dim3((unsigned)(padded_rows(c) / 128), slabs), 256, 0, s, dzp, (const uint4*)(tok ? X : Xp),
-               mtile, offsets, counts, c->H, tok ? p2f : nullptr, c->K, part);
+               mtile, offsets, counts, c->H, tok ? p2f : nullptr, c->K, kshift, part);
     MOE_LAUNCH(dwr_reduce_kernel, dim3((unsigned)c->E, slabs), 256, 0, s, part, offsets, c->H, (__nv_bfloat16*)dWr);
   } else if (dWr) {
     dim3 grid((unsigned)c->E, (unsigned)ceil_div(c->H, 256));
