@@ -965,12 +965,8 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
 // because the unpaired last M-tile of every other expert needs a second launch whose tail costs what the pairs save
 // (measured).  Debug knob, not part of the ABI: MOE_B200_PAIR=0 (never) / 1 / 2 (ragged GEMMs too).
 int pair_mode() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = getenv("MOE_B200_PAIR");
-    v = (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
-  }
-  return v;
+  const char* e = getenv("MOE_B200_PAIR");       // read per call: tests flip it inside one process
+  return (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
 }
 
 // One logical GEMM = the pair kernel over the paired M-tiles (or over everything: single group, wgrad) followed by the

@@ -215,3 +215,19 @@ def test_fused_rows_query():
     assert moe.moe_layer_rows_fused(wl.TINY) == 0
     assert moe.moe_layer_rows_fused(wl.QWEN3_SMALL) == 0
     assert moe.moe_layer_rows_fused(wl.DSV3_FP8_SMALL.replace(row_align=128)) == 0
+
+
+@pytest.mark.parametrize("pair", ["0", "2"])
+@pytest.mark.parametrize("cfg", [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128),
+                                 wl.QWEN3_SMALL.replace(name="qwen3_small_align256", row_align=256),
+                                 wl.GPTOSS_SMALL.replace(name="gptoss_small_align128", row_align=128)], ids=lambda c: c.name)
+def test_cta_pair_kernel_levels_match_oracle(cfg, pair, monkeypatch):
+    """MOE_B200_PAIR: 1 (default, the other tests) runs the weight gradients and single-group GEMMs on the cta_group::2 pair
+    kernel; 0 keeps every GEMM on the 1-CTA kernel; 2 also runs the ragged expert GEMMs as M-tile pairs (device-built
+    pair / unpaired tile lists) followed by the 1-CTA kernel over the unpaired last tiles.  With row_align = 256 every
+    tile is paired.  Same oracle, same tolerance."""
+    monkeypatch.setenv("MOE_B200_PAIR", pair)
+    inp = gc.gen_inputs(cfg)
+    lb = gc.run_gpu_layer(cfg, inp)
+    errs = gc.compare_layer(cfg, inp, lb)
+    print(cfg.name, "pair level", pair, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
