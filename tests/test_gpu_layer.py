@@ -20,6 +20,10 @@ LAYER_CASES = [
     wl.GPTOSS_SMALL.replace(name="gptoss_small_align128", row_align=128),
     wl.TINY.replace(name="tiny_bf16_align128", dtype=wl.DTYPE_BF16, row_align=128),
     wl.QWEN3_SMALL.replace(name="one_token", T=1, row_align=128),
+    # degenerate routings: a single expert (every token, weight 1), top-1 of two, and K = E (every expert for every token)
+    wl.TINY.replace(name="tiny_one_expert", E=1, K=1),
+    wl.QWEN3_SMALL.replace(name="top1_of_two", E=2, K=1, row_align=128),
+    wl.QWEN3_SMALL.replace(name="all_experts", T=300, E=4, K=4, row_align=128),
 ]
 
 
