@@ -75,7 +75,8 @@ enum moe_status {
   MOE_ERR_INVALID_ARG = -1, /* NULL where a pointer is required, non-positive size, bad enum    */
   MOE_ERR_UNSUPPORTED = -2, /* valid in principle, not implemented for this shape / dtype        */
   MOE_ERR_WORKSPACE = -3,   /* reserved                                                          */
-  MOE_ERR_CUDA = -4         /* a CUDA runtime / driver call failed (launch error, no sm_100 GPU) */
+  MOE_ERR_CUDA = -4,        /* a CUDA runtime / driver call failed (launch error, no sm_100 GPU) */
+  MOE_ERR_TOO_LARGE = -5    /* moe_permute_static_ws: the problem needs more than the built-in scratch */
 };
 
 /* Text for a status code (static storage). */
@@ -135,6 +136,25 @@ int32_t moe_route_threshold(const moe_config_t* cfg, const float* logits, const 
 int32_t moe_permute(const moe_config_t* cfg, const void* X, const int32_t* topk_idx, int32_t* counts,
                     int32_t* offsets, int32_t* perm_to_flat, int32_t* flat_to_perm, void* Xp, void* ws,
                     void* stream);
+
+/* moe_permute for callers that cannot supply `ws` because they cannot allocate device memory at all: a plug-in inside
+ * a runtime that owns the GPU's memory and passes only input / output tensors, a process that forbids cudaMalloc after
+ * start-up (it synchronises the device and can fail on a nearly full GPU), a loop that must stay clear of the allocator.
+ * Same arguments, results and limits as moe_permute minus `ws`; the scratch (the chunk histograms) is a fixed array of
+ * MOE_PERMUTE_STATIC_WS_BYTES built into the library image, so every GPU that loads libmoe_b200.so gives up that much
+ * memory until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine).
+ *   Limit: ceil(T*K / 1024) * E * 4 <= MOE_PERMUTE_STATIC_WS_BYTES, else MOE_ERR_TOO_LARGE and nothing is enqueued
+ *   (all five BASELINE.json configs need 32 KiB; T*K = 1M positions with E = 256 is the largest that fits).
+ *   First call on each device: looks up the array's device address (cudaGetSymbolAddress, with that device current)
+ *   and caches it; make that first call before any stream capture begins.
+ *   One array per GPU, shared by all calls, contents left over from the last call.  Nothing needs clearing (every entry
+ *   that is read is written first by the same call).  Calls that overlap on one GPU -- two streams, two threads -- race
+ *   on the array and corrupt each other's maps: serialise them (one stream, or events).
+ *   The GEMM tile tables moe_permute leaves in `ws` as a by-product are not produced. */
+#define MOE_PERMUTE_STATIC_WS_BYTES (1u << 20)
+int32_t moe_permute_static_ws(const moe_config_t* cfg, const void* X, const int32_t* topk_idx, int32_t* counts,
+                              int32_t* offsets, int32_t* perm_to_flat, int32_t* flat_to_perm, void* Xp,
+                              void* stream);
 
 /* R7, one grouped GEMM: for every expert e and row r in [offsets[e], offsets[e+1]):
  *   C[r, n] = sum_k A[r, k] * B[e][n, k]         A [TK_pad,Kdim], B [E,N,Kdim], C [TK_pad,N]

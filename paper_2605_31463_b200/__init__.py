@@ -14,6 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmoe_b200.so")
 
 MOE_OK, MOE_ERR_INVALID_ARG, MOE_ERR_UNSUPPORTED, MOE_ERR_WORKSPACE, MOE_ERR_CUDA = 0, -1, -2, -3, -4
+MOE_ERR_TOO_LARGE = -5
+MOE_PERMUTE_STATIC_WS_BYTES = 1 << 20   # include/moe_b200.h
 
 
 class moe_config_t(C.Structure):
@@ -63,6 +65,7 @@ _SIGNATURES = {
     "moe_layer_fwd_ex": (_I32, [_CFG] + [_P] * 14 + [C.POINTER(moe_extras_t), _P]),
     "moe_layer_bwd_ex": (_I32, [_CFG] + [_P] * 19 + [C.POINTER(moe_extras_t), _P]),
     "moe_permute": (_I32, [_CFG] + [_P] * 9),
+    "moe_permute_static_ws": (_I32, [_CFG] + [_P] * 8),
     "moe_grouped_gemm_fwd": (_I32, [_CFG, _I32, _I32] + [_P] * 8),
     "moe_grouped_gemm_bwd": (_I32, [_CFG, _I32, _I32] + [_P] * 8),
     "moe_swiglu": (_I32, [_CFG, _P, _P, _I64, _P]),
@@ -225,6 +228,17 @@ def moe_permute(cfg, X, topk_idx, counts, offsets, perm_to_flat, flat_to_perm, X
     _check(lib().moe_permute(C.byref(make_config(cfg)), _ptr(X), _ptr(topk_idx), _ptr(counts), _ptr(offsets),
                              _ptr(perm_to_flat), _ptr(flat_to_perm), _ptr(Xp), _ptr(ws), _stream(stream)),
            "moe_permute")
+
+
+def moe_permute_static_ws(cfg, X, topk_idx, counts, offsets, perm_to_flat, flat_to_perm, Xp, stream=None):
+    """moe_permute without the `ws` argument, for callers that have no way to allocate one (they are handed only input
+    and output tensors by a runtime that owns the device memory, or must not call cudaMalloc).  The scratch is a fixed
+    1 MiB array inside the library; ceil(T*K/1024)*E*4 bytes must fit in it (MoEError MOE_ERR_TOO_LARGE otherwise).
+    All calls on a GPU share that array: do not let two of them run at the same time.  Make the first call on a
+    device outside any stream capture (it looks up the array's address).  See include/moe_b200.h."""
+    _check(lib().moe_permute_static_ws(C.byref(make_config(cfg)), _ptr(X), _ptr(topk_idx), _ptr(counts), _ptr(offsets),
+                                       _ptr(perm_to_flat), _ptr(flat_to_perm), _ptr(Xp), _stream(stream)),
+           "moe_permute_static_ws")
 
 
 def moe_grouped_gemm_fwd(cfg, N, Kdim, A, B, offsets, Cout, a_scales, b_scales, ws, stream=None):

@@ -170,6 +170,7 @@ extern "C" const char* moe_status_string(int32_t status) {
     case MOE_ERR_UNSUPPORTED: return "unsupported configuration";
     case MOE_ERR_WORKSPACE: return "workspace error";
     case MOE_ERR_CUDA: return "CUDA error";
+    case MOE_ERR_TOO_LARGE: return "problem exceeds the built-in scratch (MOE_PERMUTE_STATIC_WS_BYTES) of moe_permute_static_ws";
     default: return "unknown status";
   }
 }
