@@ -89,6 +89,7 @@ inline bool dense_router_bwd(const moe_config_t* c) {
 //     replace), kept selectable with MOE_B200_FUSED_ROWS=2.
 //  0 (MOE_B200_FUSED_ROWS=0, and every other dtype / layout): w in the combine, dy = w dY from combine-backward.
 int rows_fused(const moe_config_t* c);   // layout.cu
+bool rows_fusable(const moe_config_t* c);  // the config admits levels 1 / 2 (decides the ws layout; the knob does not)
 
 // ---- byte layout of ctx / ws ---------------------------------------------------------------
 struct CtxLayout {

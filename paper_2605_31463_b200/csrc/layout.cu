@@ -41,9 +41,12 @@ int32_t layer_preflight(const moe_config_t* c, bool backward) {
   return MOE_OK;
 }
 
+bool rows_fusable(const moe_config_t* c) {
+  return c->dtype == 1 && c->H % 64 == 0 && c->F % 64 == 0 && c->row_align % 128 == 0 && n_zc(c) == 0;
+}
+
 int rows_fused(const moe_config_t* c) {
-  const bool ok = c->dtype == 1 && c->H % 64 == 0 && c->F % 64 == 0 && c->row_align % 128 == 0 && n_zc(c) == 0;
-  if (!ok) return 0;
+  if (!rows_fusable(c)) return 0;
   const char* e = getenv("MOE_B200_FUSED_ROWS");      // read per call: tests flip it inside one process
   if (e && e[0] >= '0' && e[0] <= '2') return e[0] - '0';
   return 1;
@@ -135,7 +138,9 @@ WsLayout ws_layout(const moe_config_t* c) {
   L.dzp = k.take(R * 4);
   L.dwr_part = k.take((R / 128 + 1) * H * 4);   // per-tile partial sums of dWr (fp32)
   L.dy = k.take(R * H * es);                                 // fused rows: the UNWEIGHTED gathered dY
-  if (rows_fused(c)) L.dwpart = k.take(2 * ((F + 255) / 256) * R * 4);
+  // reserved whenever the config COULD fuse, whatever MOE_B200_FUSED_ROWS says right now: every offset below must be the
+  // same for the sizing query, moe_layer_bwd and a later moe_layer_wgrad even if the knob changes between them
+  if (rows_fusable(c)) L.dwpart = k.take(2 * ((F + 255) / 256) * R * 4);
   L.dgu = k.take(R * 2 * F * es);
   L.dXp = k.take(R * H * es);
   if (Fs) {

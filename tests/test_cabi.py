@@ -96,3 +96,18 @@ def test_layer_calls_reject_unsupported_configs_before_any_launch(moe):
     fp8_unaligned = wl.DSV3_FP8_SMALL.replace(row_align=1)
     st = l.moe_layer_fwd(C.byref(moe.make_config(fp8_unaligned)), *([dummy] * 14), None)
     assert st == moe.MOE_ERR_UNSUPPORTED
+
+
+def test_ws_layout_does_not_depend_on_the_fusion_knob(moe, monkeypatch):
+    """The workspace size and every offset inside it are fixed by the config alone: MOE_B200_FUSED_ROWS may change between
+    the sizing query, moe_layer_bwd and a delayed moe_layer_wgrad without moving `dgu` / `dXp` (layout.cu)."""
+    cfg = wl.QWEN3_SMALL.replace(row_align=128)
+    seen = set()
+    for level in (None, "0", "1", "2"):
+        if level is None:
+            monkeypatch.delenv("MOE_B200_FUSED_ROWS", raising=False)
+        else:
+            monkeypatch.setenv("MOE_B200_FUSED_ROWS", level)
+        seen.add((moe.moe_workspace_bytes(cfg), moe.moe_ws_field(cfg, "dy"), moe.moe_ws_field(cfg, "dgu"),
+                  moe.moe_ws_field(cfg, "dXp")))
+    assert len(seen) == 1
