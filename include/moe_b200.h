@@ -261,7 +261,9 @@ int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const void* dY, 
 /* End-to-end step with HOST activations: copies X_host and dY_host [T,H] to the device buffers
  * X_dev / dY_dev, runs moe_layer_fwd + moe_layer_bwd, copies Y and dX back to Y_host / dX_host, all on
  * `stream` (host buffers should be pinned; returns without synchronising).  Weights, gradients, ctx,
- * ws and the staging buffers X_dev, dY_dev, Y_dev, dX_dev are device memory. */
+ * ws and the staging buffers X_dev, dY_dev, Y_dev, dX_dev are device memory.  The host steps take no moe_extras_t:
+ * a config that needs one (route_mode == 1, n_const > 0) is INVALID_ARG here; every argument check of moe_layer_fwd /
+ * moe_layer_bwd is made before the first copy is enqueued. */
 int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const void* dY_host, void* Y_host,
                             void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
                             const void* Wr, const float* bias, const void* Wg, const void* Wu, const void* Wd,

@@ -74,6 +74,30 @@ extern "C" int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int3
   return MOE_OK;
 }
 
+// Everything moe_layer_fwd / moe_layer_bwd would refuse about a host step's arguments, decided BEFORE the first copy or
+// event wait is enqueued, so that an INVALID_ARG / UNSUPPORTED host step leaves the streams (and the pipeline object)
+// untouched.  The host steps take no moe_extras_t: configs that need one (threshold routing, constant experts) are
+// rejected here; run those through moe_layer_fwd_ex / moe_layer_bwd_ex.
+static int32_t host_step_preflight(const moe_config_t* cfg, const void* Wr, const float* bias, const void* Wg,
+                                   const void* Wu, const void* Wd, const void* Wg_s, const void* Wu_s, const void* Wd_s,
+                                   const void* dWg, const void* dWu, const void* dWd, const void* dWg_s,
+                                   const void* dWu_s, const void* dWd_s, const int32_t* topk_idx, const float* topk_w,
+                                   const void* ctx, const void* ws) {
+  MOE_CHECK(layer_preflight(cfg, true));
+  if (!Wr || !topk_idx || !topk_w || !ctx || !ws) return MOE_ERR_INVALID_ARG;
+  if (cfg->has_bias && !bias) return MOE_ERR_INVALID_ARG;
+  if (cfg->route_mode == 1 || cfg->n_const > 0) return MOE_ERR_INVALID_ARG;      // need moe_extras_t
+  const bool shared = cfg->F_shared > 0;
+  const bool cached = cfg->dtype == 2 && !Wg && !Wu && !Wd;                      // FP8 weight cache in ctx
+  if (!cached && (!Wg || !Wu || !Wd)) return MOE_ERR_INVALID_ARG;
+  if (shared && !cached && (!Wg_s || !Wu_s || !Wd_s)) return MOE_ERR_INVALID_ARG;
+  const bool wgrad = dWg || dWu || dWd;
+  if (wgrad && !(dWg && dWu && dWd)) return MOE_ERR_INVALID_ARG;
+  const bool wgrad_s = dWg_s || dWu_s || dWd_s;
+  if (wgrad_s && !(shared && dWg_s && dWu_s && dWd_s)) return MOE_ERR_INVALID_ARG;
+  return MOE_OK;
+}
+
 extern "C" int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_host, const void* dY_host, void* Y_host,
                                        void* dX_host, void* X_dev, void* dY_dev, void* Y_dev, void* dX_dev,
                                        const void* Wr, const float* bias, const void* Wg, const void* Wu,
@@ -82,7 +106,8 @@ extern "C" int32_t moe_layer_step_host(const moe_config_t* cfg, const void* X_ho
                                        int32_t* topk_idx, float* topk_w, void* ctx, void* ws, void* stream) {
   if (!cfg || !X_host || !dY_host || !Y_host || !dX_host || !X_dev || !dY_dev || !Y_dev || !dX_dev)
     return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(layer_preflight(cfg, true));
+  MOE_CHECK(host_step_preflight(cfg, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, topk_idx,
+                                topk_w, ctx, ws));
   cudaStream_t s = as_stream(stream);
   const size_t bytes = (size_t)cfg->T * cfg->H * elem_bytes(cfg);
   MOE_CUDA(cudaMemcpyAsync(X_dev, X_host, bytes, cudaMemcpyHostToDevice, s));
@@ -155,7 +180,8 @@ extern "C" int32_t moe_layer_step_host_pipelined(
   if (!pl || pl->magic != PIPE_MAGIC) return MOE_ERR_INVALID_ARG;
   if (!cfg || !X_host || !dY_host || !Y_host || !dX_host || !X_dev || !dY_dev || !Y_dev || !dX_dev || slot < 0 || slot > 1)
     return MOE_ERR_INVALID_ARG;
-  MOE_CHECK(layer_preflight(cfg, true));
+  MOE_CHECK(host_step_preflight(cfg, Wr, bias, Wg, Wu, Wd, Wg_s, Wu_s, Wd_s, dWg, dWu, dWd, dWg_s, dWu_s, dWd_s, topk_idx,
+                                topk_w, ctx, ws));
   if (current_device() != pl->device) return MOE_ERR_INVALID_ARG;   // the events belong to the device they were made on
   cudaStream_t si = as_stream(stream_in), sc = as_stream(stream_compute), so = as_stream(stream_out);
   cudaEvent_t ev_in = pl->ev[slot][0], ev_comp = pl->ev[slot][1], ev_out = pl->ev[slot][2];

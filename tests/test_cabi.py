@@ -111,3 +111,20 @@ def test_ws_layout_does_not_depend_on_the_fusion_knob(moe, monkeypatch):
         seen.add((moe.moe_workspace_bytes(cfg), moe.moe_ws_field(cfg, "dy"), moe.moe_ws_field(cfg, "dgu"),
                   moe.moe_ws_field(cfg, "dXp")))
     assert len(seen) == 1
+
+
+def test_host_step_rejects_configs_that_need_extras_before_any_copy(moe):
+    """moe_layer_step_host takes no moe_extras_t; a threshold-routing or constant-expert config must come back as
+    INVALID_ARG from the preflight.  Without a GPU any enqueued copy would fail with MOE_ERR_CUDA instead, so the status
+    also proves that nothing was enqueued (api.cu)."""
+    l = moe.lib()
+    dummy = (C.c_int32 * 4)()
+    p = C.cast(dummy, C.c_void_p)
+    args = [p] * 27 + [None]                                      # 27 non-NULL pointers + stream
+    for cfg in (wl.TINY.replace(score_fn=1, route_mode=1), wl.TINY.replace(n_const=1)):
+        st = l.moe_layer_step_host(C.byref(moe.make_config(cfg)), *args)
+        assert st == moe.MOE_ERR_INVALID_ARG, moe.status_string(st)
+    # a missing weight pointer is caught there as well (Wg is the 11th pointer)
+    bad = list(args)
+    bad[10] = None
+    assert l.moe_layer_step_host(C.byref(moe.make_config(wl.TINY)), *bad) == moe.MOE_ERR_INVALID_ARG
