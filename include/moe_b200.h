@@ -16,9 +16,11 @@
  *  - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream);
  *    calls return without synchronising.  Per-expert counts never visit the host.
  *  - Row-major, innermost dimension contiguous, base pointers 16-byte aligned.
- *  - Return value: MOE_OK or a negative moe_status.  INVALID_ARG and UNSUPPORTED are decided before the first
- *    launch (the layer calls check every stage's limits up front), so on those nothing has been enqueued and
- *    no output buffer has been touched; MOE_ERR_CUDA (a failed launch or runtime call) can occur mid-way.
+ *  - Return value: MOE_OK or a negative moe_status.  INVALID_ARG, and UNSUPPORTED for every limit this header lists
+ *    (the config checks, E <= 1024, K <= 32, n_group <= 32, FP8 needs row_align % 128 == 0), are decided before the
+ *    first launch, so on those nothing has been enqueued and no output buffer has been touched.  MOE_ERR_CUDA (a failed
+ *    launch or runtime call) can occur mid-way, and so can an UNSUPPORTED that only a later stage can discover (the
+ *    driver refusing a tensor map for an exotic leading dimension): after either, ctx / ws / outputs are undefined.
  *    No exceptions, no aborts, no printing.  Inputs must be finite.
  *  - Activation / weight element type follows cfg->dtype: 0 = fp32, 1 = bf16, 2 = bf16 I/O with
  *    e4m3 block-scaled expert GEMMs.  Logits, gating weights and their gradients are always fp32.

@@ -50,8 +50,11 @@ inline int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 inline int64_t ceil_div(int64_t x, int64_t a) { return (x + a - 1) / a; }
 
 int32_t validate(const moe_config_t* c);
-// Every limit of every stage of moe_layer_fwd / bwd / wgrad for this config, checked BEFORE the first launch, so that
-// an UNSUPPORTED layer call enqueues nothing (include/moe_b200.h conventions).  Includes validate().
+// The limits include/moe_b200.h lists for moe_layer_fwd / bwd / wgrad (validate() + the routing kernel's E, K, n_group
+// bounds + FP8 row alignment), checked BEFORE the first launch so that those UNSUPPORTED cases enqueue nothing.  It does
+// not mirror every shape predicate of tc_gemm / fp8_gemm: the layer picks the CUDA-core GEMM for shapes the tensor-core
+// path does not take, and a tensor-map creation failure inside a stage can still surface after earlier stages ran.
+// `backward` is unused today (both directions share the limits).
 int32_t layer_preflight(const moe_config_t* c, bool backward);
 
 // Lazily filled per-device caches (function attributes, SM counts) are indexed by the CURRENT device, so a process

@@ -52,6 +52,28 @@ __global__ void __launch_bounds__(CHUNK_WARPS * 32) hist_kernel(const int32_t* _
   }
 }
 
+// Phase 1b, only for many chunks (nchunks > PREFIX_MIN_CHUNKS): turn each expert's column of chunk counts into an
+// INCLUSIVE prefix over chunks, in place, so that phase 2 reads two entries per expert instead of the whole column
+// (otherwise every one of the nchunks CTAs walks all nchunks rows: O(nchunks^2 E) loads, 1 GB of L2 reads at T*K = 1M).
+// One CTA per expert, strided block scan with a running carry.
+constexpr int PREFIX_MIN_CHUNKS = 256;
+__global__ void __launch_bounds__(1024) hist_prefix_kernel(int32_t* __restrict__ hist, int E, int nchunks) {
+  __shared__ int32_t wsum[32];
+  __shared__ int32_t s_carry;
+  const int e = blockIdx.x;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  for (int c0 = 0; c0 < nchunks; c0 += 1024) {
+    const int c = c0 + threadIdx.x;
+    const int v = c < nchunks ? hist[(size_t)c * E + e] : 0;
+    const int incl = block_incl_scan_1024(v, wsum) + s_carry;
+    if (c < nchunks) hist[(size_t)c * E + e] = incl;
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = incl;
+    __syncthreads();
+  }
+}
+
 // Phase 2: scan + scatter in one launch (1024 threads per chunk CTA).  Every CTA rebuilds what it needs from the chunk
 // histograms (E x nchunks ints, L2-resident): thread e sums expert e's column -> counts, aligned exclusive offsets by a block
 // scan, and the chunk's base row of expert e = offsets[e] + positions of e in earlier chunks.  CTA 0 also publishes counts,
@@ -63,7 +85,7 @@ __global__ void __launch_bounds__(1024) scan_scatter_kernel(const int32_t* __res
                                                             int32_t* __restrict__ counts, int32_t* __restrict__ offsets,
                                                             int32_t* __restrict__ mtile, int32_t* __restrict__ plist,
                                                             int32_t* __restrict__ olist, int32_t* __restrict__ p2f,
-                                                            int32_t* __restrict__ f2p, int64_t rows_cap) {
+                                                            int32_t* __restrict__ f2p, int64_t rows_cap, int prefixed) {
   extern __shared__ int32_t sm[];          // [E] chunk bases, then [CHUNK_WARPS][E] per-warp histograms
   __shared__ int32_t wsum[32];
   __shared__ int32_t s_end;
@@ -72,10 +94,15 @@ __global__ void __launch_bounds__(1024) scan_scatter_kernel(const int32_t* __res
   const int e = threadIdx.x;
   int cnt = 0, before = 0;
   if (e < E) {
-    for (int c = 0; c < nchunks; ++c) {
-      const int h = hist[(size_t)c * E + e];
-      if (c < (int)blockIdx.x) before += h;
-      cnt += h;
+    if (prefixed) {   // hist holds inclusive prefixes over chunks (hist_prefix_kernel)
+      cnt = hist[(size_t)(nchunks - 1) * E + e];
+      before = blockIdx.x > 0 ? hist[(size_t)(blockIdx.x - 1) * E + e] : 0;
+    } else {
+      for (int c = 0; c < nchunks; ++c) {
+        const int h = hist[(size_t)c * E + e];
+        if (c < (int)blockIdx.x) before += h;
+        cnt += h;
+      }
     }
   }
   const int a = row_align < 1 ? 1 : row_align;
@@ -139,11 +166,13 @@ int32_t build_maps(const moe_config_t* c, const int32_t* idx, int32_t* counts, i
   if (c->E > 1024) return MOE_ERR_UNSUPPORTED;
   const size_t smem = (size_t)CHUNK_WARPS * c->E * sizeof(int32_t);
   MOE_LAUNCH(hist_kernel, nchunks, CHUNK_WARPS * 32, smem, s, idx, TK, c->E, hist);
+  const int prefixed = nchunks > PREFIX_MIN_CHUNKS;
+  if (prefixed) MOE_LAUNCH(hist_prefix_kernel, c->E, 1024, 0, s, hist, c->E, nchunks);
   int32_t* mt = (c->row_align % 128 == 0) ? mtile_expert : nullptr;
   const int64_t R = padded_rows(c);
   MOE_LAUNCH(scan_scatter_kernel, nchunks, 1024, smem + (size_t)c->E * sizeof(int32_t), s, idx, TK, c->E, e_ffn(c), c->row_align,
              hist, nchunks, counts, offsets, mt, mt ? mt + tile_plist_off(R) : nullptr, mt ? mt + tile_olist_off(R) : nullptr,
-             p2f, f2p, R);
+             p2f, f2p, R, prefixed);
   return MOE_OK;
 }
 

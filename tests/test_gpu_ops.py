@@ -70,7 +70,9 @@ def test_route_hand_made_ties(env):
 
 PERM_CASES = [wl.TINY, wl.QWEN3_SMALL, wl.GPTOSS_SMALL, wl.DSV3_SMALL, wl.TINY.replace(name="t1", T=1),
               wl.TINY.replace(name="t1025", T=1025, K=3), wl.QWEN3.replace(name="qwen3_full_perm"),
-              wl.GPTOSS.replace(name="gptoss_full_perm")]
+              wl.GPTOSS.replace(name="gptoss_full_perm"),
+              # > 256 chunks of 1024 positions: the chunk histograms are prefix-summed by their own launch (permute.cu)
+              wl.QWEN3.replace(name="many_chunks", T=40001, H=64, F=64)]
 
 
 @pytest.mark.parametrize("cfg", PERM_CASES, ids=lambda c: c.name)
