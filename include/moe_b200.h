@@ -59,6 +59,15 @@ typedef struct moe_config_t {
                                   Wg, Wu, Wd and their gradients hold E - n_zero - n_copy - n_const experts    */
   float aux_coef;              /* auxiliary load-balancing loss coefficient (A1); 0 = off    */
   float aux_zc_weight;         /* weight of the zero-computation experts in the balance term    */
+  /* ---- kernel-variant selectors.  All 0 = the library's defaults (the measured, documented path).  The library reads
+   * NO environment variables; these fields are the only way to reach the non-default variants, which exist so that the
+   * tests can hold every variant to the same oracle.  Value v > 0 forces level v - 1. ---- */
+  int32_t opt_rows_fused;      /* levels 0 / 1 / 2 of moe_layer_rows_fused (ignored where the config cannot fuse)      */
+  int32_t opt_pair;            /* cta_group::2 pair kernel: level 0 never, 1 weight gradients + single-group GEMMs
+                                  (default), 2 ragged expert GEMMs as M-tile pairs too                                 */
+  int32_t opt_fp8_wide;        /* FP8 128 x 256 tiles: level 0 never, 1 plain-epilogue GEMMs (default), 2 all modes    */
+  int32_t opt_fp8_fused_quant; /* Q-a / Q-dgu in the GEMM epilogues: level 0 off, 1 on (default: on iff
+                                  fp8_scale_mode == 1)                                                                 */
 } moe_config_t;
 
 /* Optional inputs / outputs of the widened rows, passed to moe_layer_fwd_ex / moe_layer_bwd_ex (NULL members that the
@@ -94,13 +103,13 @@ int64_t moe_padded_rows(const moe_config_t* cfg);
 /* How moe_layer_fwd / bwd / wgrad fold the routing weight and the permutation into the grouped GEMMs for this config
  * (< 0: invalid config).  PAPER.md:116 ("fused ... token scatter"); BASELINE.json north_star (3) "routing-weight scaling
  * fused into the epilogues".
- *  0  nothing fused (fp32, FP8, unaligned groups, zero-computation experts; or MOE_B200_FUSED_ROWS=0): w is applied in the
+ *  0  nothing fused (fp32, FP8, unaligned groups, zero-computation experts; or cfg->opt_rows_fused = 1): w is applied in the
  *     combine, the backward starts with a combine-backward pass writing dy = w dY and dw.
  *  1  (default for bf16 with H, F multiples of 64 and row_align a multiple of 128): the routing weight is applied in the
  *     GEMM-1 epilogue (ctx "a" holds w_r a_r, ctx "y" holds w_r y_r, the combine is a plain sum over the K rows) and in the
  *     dgrad-down epilogue, which also produces dw[t,j] = <da_r, a_r> (= <dY_t, y_r>, R8).  The combine-backward pass is
  *     replaced by a plain row gather of dY: ws "dy" holds the UNWEIGHTED rows of dY, y is not read by the backward.
- *  2  (MOE_B200_FUSED_ROWS=2) as 1, and GEMM-1 gathers the rows of X, dgrad-down the rows of dY, inside the kernel (TMA
+ *  2  (cfg->opt_rows_fused = 3) as 1, and GEMM-1 gathers the rows of X, dgrad-down the rows of dY, inside the kernel (TMA
  *     tile::gather4 through perm_to_flat), each writing the row-grouped copy ("Xp", "dy") that the weight gradients contract
  *     over as a by-product of its staged tiles: no row-mover pass at all.
  * The layer's results (Y, dX, dW*, dWr, topk_*) mean the same in all three.  The stand-alone moe_permute /

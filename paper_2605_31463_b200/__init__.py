@@ -25,7 +25,9 @@ class moe_config_t(C.Structure):
                 ("has_bias", C.c_int32), ("F_shared", C.c_int32), ("dtype", C.c_int32),
                 ("fp8_scale_mode", C.c_int32), ("row_align", C.c_int32),
                 ("route_mode", C.c_int32), ("n_zero", C.c_int32), ("n_copy", C.c_int32), ("n_const", C.c_int32),
-                ("aux_coef", C.c_float), ("aux_zc_weight", C.c_float)]
+                ("aux_coef", C.c_float), ("aux_zc_weight", C.c_float),
+                ("opt_rows_fused", C.c_int32), ("opt_pair", C.c_int32), ("opt_fp8_wide", C.c_int32),
+                ("opt_fp8_fused_quant", C.c_int32)]
 
 
 class moe_extras_t(C.Structure):
@@ -40,7 +42,7 @@ def make_config(cfg) -> moe_config_t:
     """Build the C struct from any object carrying the moe_config_t field names (e.g. workloads.MoEConfig)."""
     if isinstance(cfg, moe_config_t):
         return cfg
-    return moe_config_t(**{f: getattr(cfg, f) for f in CONFIG_FIELDS})
+    return moe_config_t(**{f: getattr(cfg, f, 0) if f.startswith("opt_") else getattr(cfg, f) for f in CONFIG_FIELDS})
 
 
 class MoEError(RuntimeError):

@@ -1,6 +1,7 @@
 """Build libmoe_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -13,6 +14,38 @@ LIB = os.path.join(HERE, "libmoe_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr", "-Xptxas", "-v"]
+
+
+HASH_FILE = LIB + ".hash"
+
+
+def source_hash() -> str:
+    """Identity of what the library is built from: every file of csrc/, the public header and the nvcc flags.  Stored
+    beside the .so by build(); a .so whose stored hash differs from the tree's (a stale binary that travelled to the GPU
+    box, an edit that kept an old mtime) is rebuilt from scratch instead of being trusted."""
+    h = hashlib.sha256()
+    files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h"))]
+    files.append(os.path.join(HERE, "..", "include", "moe_b200.h"))
+    for f in files:
+        h.update(os.path.basename(f).encode() + b"\0")
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    h.update(" ".join(FLAGS).encode())
+    return h.hexdigest()[:16]
+
+
+def built_hash():
+    """Hash recorded by the build that produced the in-tree .so (None: no .so or no record)."""
+    if not (os.path.exists(LIB) and os.path.exists(HASH_FILE)):
+        return None
+    with open(HASH_FILE) as fh:
+        return fh.read().strip()
+
+
+def build_id() -> dict:
+    """What bench.py and smoke() print so that a number can be tied to the source it was measured on."""
+    have = built_hash()
+    return {"source_hash": source_hash(), "library_hash": have, "library_matches_tree": have == source_hash()}
 
 
 def sources():
@@ -28,6 +61,9 @@ def _stale(out, deps):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    want = source_hash()
+    if built_hash() != want:
+        force = True            # never reuse objects or a .so that were not built from exactly this tree and these flags
     hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     hdrs.append(os.path.join(HERE, "..", "include", "moe_b200.h"))
     jobs = []
@@ -56,6 +92,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         r = subprocess.run([NVCC, "-shared", "-o", LIB] + objs + ["-cudart", "static"], capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("link failed:\n" + r.stdout + r.stderr)
+        with open(HASH_FILE, "w") as fh:
+            fh.write(want + "\n")
     return LIB
 
 

@@ -21,7 +21,7 @@ extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int3
     MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
     F8Call c;
     memset(&c, 0, sizeof(c));
-    c.mode = F8_FWD; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.mtile = mtile;
+    c.mode = F8_FWD; c.opt_wide = cfg->opt_fp8_wide; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.mtile = mtile;
     c.A = (const uint8_t*)A; c.lda = Kdim; c.a_scales = (const float*)a_scales;
     c.B0 = (const uint8_t*)B; c.b0_scales = (const float*)b_scales; c.b_rows = N; c.b_cols = Kdim; c.N = N;
     c.out0 = C; c.ld0 = N;
@@ -31,7 +31,7 @@ extern "C" int32_t moe_grouped_gemm_fwd(const moe_config_t* cfg, int32_t N, int3
     MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
     TcCall c;
     memset(&c, 0, sizeof(c));
-    c.mode = TC_FWD; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    c.mode = TC_FWD; c.opt_pair = cfg->opt_pair; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
     c.plist = mtile + tile_plist_off(c.rows_cap); c.olist = mtile + tile_olist_off(c.rows_cap);
     c.A = A; c.lda = Kdim; c.B0 = B; c.b_rows = N; c.b_cols = Kdim; c.N = N; c.Kd = Kdim; c.out0 = C; c.ld0 = N;
     const int32_t st = tc_gemm(c, s);
@@ -54,7 +54,7 @@ extern "C" int32_t moe_grouped_gemm_bwd(const moe_config_t* cfg, int32_t N, int3
     MOE_CHECK(tc_prepare_tiles(offsets, cfg->E, padded_rows(cfg), mtile, s));
     TcCall c;
     memset(&c, 0, sizeof(c));
-    c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
+    c.opt_pair = cfg->opt_pair; c.E = cfg->E; c.rows_cap = padded_rows(cfg); c.offsets = offsets; c.mtile = mtile;
     c.plist = mtile + tile_plist_off(c.rows_cap); c.olist = mtile + tile_olist_off(c.rows_cap);
     if (dA) {   // dA = dC B[e]: contraction over B's rows
       c.mode = TC_DGRAD; c.A = dC; c.lda = N; c.B0 = B; c.B1 = nullptr; c.b_rows = N; c.b_cols = Kdim; c.N = Kdim;

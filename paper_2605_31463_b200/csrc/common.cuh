@@ -89,8 +89,8 @@ inline bool dense_router_bwd(const moe_config_t* c) {
 //  2: as 1, and GEMM-1 / dgrad-down gather their A rows from the token-major X / dY themselves (TMA tile::gather4 through
 //     perm_to_flat, gather-warp kernel variants), writing Xp / dy as a by-product of the staged tiles: no row-mover pass at
 //     all.  Measured slower than 1 (the by-product stores cost the GEMMs more than the passes they
-//     replace), kept selectable with MOE_B200_FUSED_ROWS=2.
-//  0 (MOE_B200_FUSED_ROWS=0, and every other dtype / layout): w in the combine, dy = w dY from combine-backward.
+//     replace), kept selectable with cfg->opt_rows_fused = 3.
+//  0 (cfg->opt_rows_fused = 1, and every other dtype / layout): w in the combine, dy = w dY from combine-backward.
 int rows_fused(const moe_config_t* c);   // layout.cu
 bool rows_fusable(const moe_config_t* c);  // the config admits levels 1 / 2 (decides the ws layout; the knob does not)
 

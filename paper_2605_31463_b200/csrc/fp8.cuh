@@ -56,6 +56,7 @@ enum F8Mode { F8_FWD = 0, F8_FWD_SWIGLU = 1, F8_DGRAD = 2, F8_DGRAD_SWIGLU = 3 }
 
 struct F8Call {
   int mode;
+  int opt_wide;            // moe_config_t::opt_fp8_wide (0 = default level 1)
   int E;
   int64_t rows_cap;        // height of the row-grouped buffers
   const int32_t* mtile;    // device {n_tiles, expert of tile 0, ...} or nullptr: one group of rows_cap rows

@@ -780,10 +780,9 @@ int32_t launch_wide(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorM
 // 128 x 256 tiles when the output width allows.  Default (1): the plain-epilogue GEMMs (gemm2, dgrad gate/up: configs[3]
 // 1.46 -> 1.16 ms, 2.71 -> 2.51 ms).  The fused-SwiGLU modes run on the wide kernel too (parity-tested) but slower (gemm1
 // 2.66 -> 2.86 ms, dgrad-down 1.67 -> 1.78 ms): their long epilogues are not overlapped with the next tile's main loop, and
-// two TMEM buffers give the MMAs less slack than four.  MOE_B200_FP8_WIDE = 0 (never) / 1 / 2 (all modes); debug knob.
-bool use_wide(int N, bool swiglu) {
-  const char* e = getenv("MOE_B200_FP8_WIDE");
-  const int level = (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
+// two TMEM buffers give the MMAs less slack than four.  moe_config_t::opt_fp8_wide: level 0 (never) / 1 / 2 (all modes).
+bool use_wide(const F8Call& c, int N, bool swiglu) {
+  const int level = c.opt_wide ? c.opt_wide - 1 : 1;
   return level > (swiglu ? 1 : 0) && N % WBN == 0;
 }
 
@@ -825,7 +824,7 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
     case F8_FWD: {
       if (c.lda != c.b_cols || c.N != c.b_rows) return MOE_ERR_INVALID_ARG;
       p.nkb = c.b_cols / BK;
-      const bool wide = use_wide(c.N, false);
+      const bool wide = use_wide(c, c.N, false);
       p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, wide ? WBN : BN)) return MOE_ERR_UNSUPPORTED;
@@ -835,7 +834,7 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
     case F8_FWD_SWIGLU: {
       if (!c.B1 || !c.b1_scales || !c.out1 || c.lda != c.b_cols || c.F != c.b_rows || (c.ld1 & 7)) return MOE_ERR_INVALID_ARG;
       p.nkb = c.b_cols / BK;
-      const bool wide = use_wide(2 * c.F, true);          // a wide tile = 128 gate + 128 up columns: F is a multiple of 128 already
+      const bool wide = use_wide(c, 2 * c.F, true);          // a wide tile = 128 gate + 128 up columns: F is a multiple of 128 already
       p.n_tiles = c.F / ((wide ? WBN : BN) / 2);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BK, (wide ? WBN : BN) / 2)) return MOE_ERR_UNSUPPORTED;
@@ -849,7 +848,7 @@ int32_t fp8_gemm(const F8Call& c, cudaStream_t s) {
       if (c.N != c.b_cols || c.lda != (split ? 2 : 1) * c.b_rows) return MOE_ERR_INVALID_ARG;
       p.kb_split = c.b_rows / BK;
       p.nkb = split ? 2 * p.kb_split : p.kb_split;
-      const bool wide = use_wide(c.N, c.mode == F8_DGRAD_SWIGLU);
+      const bool wide = use_wide(c, c.N, c.mode == F8_DGRAD_SWIGLU);
       p.n_tiles = c.N / (wide ? WBN : BN);
       if (!tc_make_map(&ta, 1, c.A, c.lda, c.rows_cap, c.lda, BK, BM)) return MOE_ERR_UNSUPPORTED;
       if (!tc_make_map(&tb0, 1, c.B0, c.b_cols, wrows, c.b_cols, BN, BK)) return MOE_ERR_UNSUPPORTED;

@@ -2,8 +2,8 @@
 //
 // One persistent, warp-specialised kernel template serves every expert GEMM of the layer (SURVEY.md §8a
 // a5, a6, a9..a12): warp 0 = TMA producer, warp 1 = MMA issuer (one elected thread, tcgen05.mma
-// cta_group::1, M=128 x N=256 x K=16 per instruction), warps 2..5 = epilogue (tcgen05.ld from a
-// double-buffered 2 x 256-column TMEM accumulator).  Operands are staged by TMA into 128-byte-swizzled
+// cta_group::1, M=128 x N=256 x K=16 per instruction), warps 2..9 = epilogue (EPI_WARPS = 8, two per TMEM lane group,
+// each taking every other 64-column chunk; tcgen05.ld from a double-buffered 2 x 256-column TMEM accumulator).  Operands are staged by TMA into 128-byte-swizzled
 // shared memory, 4 stages of (128 x 64 A tile + 256 x 64 B tile) = 192 KB.  The tile schedule is
 // computed on the device from the per-expert row offsets (shapes are data dependent; the
 // counts never visit the host): a 128-row M-tile belongs to exactly one expert because expert groups
@@ -963,11 +963,8 @@ int32_t launch(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorMap& b
 // Which launches use the CTA-pair kernel.  Default 1: the weight gradients (no ragged dimension: every 256 x 256 tile
 // is a full pair tile) and single-group GEMMs (shared expert, router); the ragged expert GEMMs stay on the 1-CTA kernel
 // because the unpaired last M-tile of every other expert needs a second launch whose tail costs what the pairs save
-// (measured).  Debug knob, not part of the ABI: MOE_B200_PAIR=0 (never) / 1 / 2 (ragged GEMMs too).
-int pair_mode() {
-  const char* e = getenv("MOE_B200_PAIR");       // read per call: tests flip it inside one process
-  return (e && e[0] >= '0' && e[0] <= '2') ? e[0] - '0' : 1;
-}
+// (measured).  Selected by moe_config_t::opt_pair: level 0 (never) / 1 / 2 (ragged GEMMs too).
+int pair_mode(const TcCall& c) { return c.opt_pair ? c.opt_pair - 1 : 1; }
 
 // One logical GEMM = the pair kernel over the paired M-tiles (or over everything: single group, wgrad) followed by the
 // 1-CTA kernel over the unpaired M-tiles.  With `pl == nullptr` (no pair table) the 1-CTA kernel runs all tiles.
@@ -977,7 +974,7 @@ int32_t launch_both(const CUtensorMap& a, const CUtensorMap& b0, const CUtensorM
                     const CUtensorMap* cp = nullptr) {
   const int64_t max_mtiles = ceil_div(c.rows_cap, BM);
   const bool grouped = c.mtile != nullptr;
-  if (pair_mode() == 0 || p.gat || (grouped && (pair_mode() < 2 || !c.plist || !c.olist))) {   // gathered A: 1-CTA kernel
+  if (pair_mode(c) == 0 || p.gat || (grouped && (pair_mode(c) < 2 || !c.plist || !c.olist))) {   // gathered A: 1-CTA kernel
     p.tlist = nullptr;
     return launch<MODE, false>(a, b0, b1, o, p, max_mtiles * p.n_tiles, s, o2, cp);
   }
@@ -1109,7 +1106,7 @@ int32_t tc_gemm(const TcCall& c, cudaStream_t s) {
       // rows_cap counts 127 padding rows per expert) and an output height that 256-row tiles cover without extra padding.
       // Measured: configs[1] 690 -> 625 us; configs[2] (128 rows per expert: 2 k-blocks per 64 KB of
       // output per CTA, write-bound) 8.04 -> 8.75 ms and configs[4] (2880 = 11.25 x 256) 4.2 -> 4.5 ms, so those stay 1-CTA.
-      const bool pair = pair_mode() > 0 && (c.mtile == nullptr || c.rows_cap >= 384 * (int64_t)c.E) &&
+      const bool pair = pair_mode(c) > 0 && (c.mtile == nullptr || c.rows_cap >= 384 * (int64_t)c.E) &&
                         ceil_div(c.M, 2 * BM) * 2 == ceil_div(c.M, BM);
       p.m_tiles = (int)ceil_div(c.M, pair ? 2 * BM : BM);
       p.n_tiles = (int)ceil_div(c.N, BN);

@@ -17,6 +17,7 @@ enum TcMode { TC_FWD = 0, TC_FWD_SWIGLU = 1, TC_DGRAD = 2, TC_DGRAD_SWIGLU = 3, 
 
 struct TcCall {
   int mode;
+  int opt_pair;            // moe_config_t::opt_pair (0 = default level 1)
   int E;                   // groups
   int64_t rows_cap;        // height of the row-grouped buffers (TMA bound; rows >= it read as zero)
   const int32_t* counts;   // [E] device or nullptr: real rows per group (WGRAD trims its contraction to them)

@@ -30,7 +30,12 @@ struct FfnGroup {
   int64_t g_rows = 0;
   const float* roww = nullptr;
   float* dwpart = nullptr;
+  int opt_pair = 0, opt_wide = 0, opt_fq = 0;   // moe_config_t::opt_pair / opt_fp8_wide / opt_fp8_fused_quant
 };
+
+inline void set_opts(FfnGroup& g, const moe_config_t* c) {
+  g.opt_pair = c->opt_pair; g.opt_wide = c->opt_fp8_wide; g.opt_fq = c->opt_fp8_fused_quant;
+}
 
 namespace {
 
@@ -48,6 +53,7 @@ TcCall tc_base(const FfnGroup& g, int mode) {
   TcCall c;
   memset(&c, 0, sizeof(c));
   c.mode = mode;
+  c.opt_pair = g.opt_pair;
   c.E = g.E;
   c.rows_cap = g.rows_cap;
   c.offsets = g.offsets;
@@ -171,10 +177,9 @@ struct Fp8Bufs {
 // (tests/test_gpu_fp8.py).  With power-of-two scales the epilogue quantises by an exact multiplication and is the
 // default; with fp32 scales (mode 0) every code needs an IEEE division on the promotion warps' critical path, which costs
 // the two GEMMs more (+0.55 / +0.76 ms on configs[3]) than the two HBM passes it removes (-0.65 ms), so the stand-alone
-// passes stay the default there.  MOE_B200_FP8_FUSED_QUANT=0/1 forces either (debug knob, not part of the ABI).
-bool fused_quant(int scale_mode) {
-  const char* e = getenv("MOE_B200_FP8_FUSED_QUANT");     // read per call: tests flip it inside one process
-  if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
+// passes stay the default there.  moe_config_t::opt_fp8_fused_quant = 1 / 2 forces off / on.
+bool fused_quant(const FfnGroup& g, int scale_mode) {
+  if (g.opt_fq) return g.opt_fq == 2;
   return scale_mode == 1;
 }
 
@@ -182,6 +187,7 @@ F8Call f8_base(const FfnGroup& g, int mode) {
   F8Call c;
   memset(&c, 0, sizeof(c));
   c.mode = mode;
+  c.opt_wide = g.opt_wide;
   c.E = g.E;
   c.rows_cap = g.rows_cap;
   c.mtile = g.mtile;
@@ -193,7 +199,7 @@ int32_t ffn_fwd_fp8(const FfnGroup& g, const Fp8Bufs& q, void* gu, void* a, void
   F8Call c = f8_base(g, F8_FWD_SWIGLU);   // gu = [Q(X) Q(Wg)^T | Q(X) Q(Wu)^T], a = silu(g) * u
   c.A = q.Aq; c.lda = g.H; c.a_scales = q.Aq_s; c.B0 = q.Wgq; c.b0_scales = q.Wgq_s; c.B1 = q.Wuq; c.b1_scales = q.Wuq_s;
   c.b_rows = g.F; c.b_cols = g.H; c.N = g.F; c.out0 = gu; c.ld0 = 2 * g.F; c.out1 = a; c.ld1 = g.F;
-  const bool fused = fused_quant(q.mode);
+  const bool fused = fused_quant(g, q.mode);
   if (fused) { c.q_codes = q.aq; c.q_scales = q.aq_s; c.q_mode = q.mode; }   // Q-a on the bf16 a, in the epilogue
   MOE_CHECK(fp8_gemm(c, s));
   prof_mark(g.st_fwd1, s);
@@ -215,7 +221,7 @@ int32_t ffn_bwd_fp8(const FfnGroup& g, const Fp8Bufs& q, const void* dy, const v
   F8Call c = f8_base(g, F8_DGRAD_SWIGLU);  // dgu = swiglu'(gu) * w_r * (Q(dY)[t_r] Q(Wd)[e])
   c.A = q.dyq; c.lda = g.H; c.a_scales = q.dyq_s; c.B0 = q.Wdq; c.b0_scales = q.Wdq_s; c.b_rows = g.H; c.b_cols = g.F;
   c.N = g.F; c.gu = gu; c.ldgu = 2 * g.F; c.out0 = dgu; c.ld0 = 2 * g.F; c.p2f = q.p2f; c.w = q.w;
-  const bool fused = fused_quant(q.mode);
+  const bool fused = fused_quant(g, q.mode);
   if (fused) { c.q_codes = q.dguq; c.q_scales = q.dguq_s; c.q_mode = q.mode; }   // Q-dgu in the epilogue
   MOE_CHECK(fp8_gemm(c, s));
   prof_mark(g.st_bwd1, s);
@@ -317,6 +323,7 @@ extern "C" int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, cons
   FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  set_opts(g, cfg);
   if (fused) { g.gidx = p2f; g.gK = cfg->K; g.g_rows = cfg->T; g.roww = topk_w; }
   if (fused == 2) g.tok_in = X;
   Fp8Bufs q, qs;
@@ -357,6 +364,7 @@ extern "C" int32_t moe_layer_fwd_ex(const moe_config_t* cfg, const void* X, cons
     int32_t* off_s = offsets + cfg->E + 1;
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
+    set_opts(gs, cfg);
     if (fp8)
       MOE_CHECK(ffn_fwd_fp8(gs, qs, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ctx, C.y_s), s));
     else
@@ -426,6 +434,7 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
   FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, counts,
              (cfg->row_align % 128 == 0) ? mtile : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  set_opts(g, cfg);
   if (fused) { g.gidx = p2f; g.gK = cfg->K; g.g_rows = cfg->T; g.roww = w; g.dwpart = at<float>(ws, W.dwpart); }
   if (fused == 2) g.tok_in = dY;
   Fp8Bufs q, qs;
@@ -475,6 +484,7 @@ extern "C" int32_t moe_layer_bwd_ex(const moe_config_t* cfg, const void* dY, con
     const int32_t* off_s = offsets + cfg->E + 1;
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, off_s, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
+    set_opts(gs, cfg);
     if (fp8)
       MOE_CHECK(ffn_bwd_fp8(gs, qs, dY, X, at<char>(ctx, C.gu_s), at<char>(ctx, C.a_s), at<char>(ws, W.dgu_s),
                             at<char>(ws, W.dXs), dWg_s, dWu_s, dWd_s, s));
@@ -515,12 +525,14 @@ extern "C" int32_t moe_layer_wgrad(const moe_config_t* cfg, const void* X, const
   FfnGroup g{cfg->dtype, e_ffn(cfg), cfg->H, cfg->F, padded_rows(cfg), offsets, at<int32_t>(ctx, C.counts),
              (cfg->row_align % 128 == 0) ? at<int32_t>(ctx, C.mtile) : nullptr, cfg->row_align,
              ST_GEMM1_SWIGLU, ST_GEMM2, ST_DGRAD_DOWN_SWIGLU, ST_DGRAD_GATEUP, ST_WGRAD};
+  set_opts(g, cfg);
   prof_mark(ST_BEGIN, s);
   MOE_CHECK(ffn_wgrad(g, at<char>(ws, W.dy), at<char>(ctx, C.Xp), at<char>(ctx, C.a), at<char>(ws, W.dgu), dWg, dWu, dWd,
                       accumulate_fp32 ? 1 : 0, s));
   if (wgrad_s) {
     FfnGroup gs{cfg->dtype, 1, cfg->H, cfg->F_shared, cfg->T, offsets + cfg->E + 1, nullptr, nullptr, 1,
                 ST_SHARED_FWD, ST_SHARED_FWD, ST_SHARED_BWD, ST_SHARED_BWD, ST_SHARED_BWD};
+    set_opts(gs, cfg);
     MOE_CHECK(ffn_wgrad(gs, dY, X, at<char>(ctx, C.a_s), at<char>(ws, W.dgu_s), dWg_s, dWu_s, dWd_s, accumulate_fp32 ? 1 : 0, s));
   }
   return MOE_OK;

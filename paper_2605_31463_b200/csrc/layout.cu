@@ -1,5 +1,4 @@
 // Config validation, ctx / ws byte layouts and the small query entry points of the C ABI.
-#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -28,6 +27,9 @@ int32_t validate(const moe_config_t* c) {
   if (c->route_mode == 1 && (c->score_fn != 1 || c->n_group != 1 || c->has_bias)) return MOE_ERR_INVALID_ARG;
   if (n_zc(c) >= c->E) return MOE_ERR_INVALID_ARG;              // at least one FFN expert
   if (!(c->aux_coef == c->aux_coef) || !(c->aux_zc_weight == c->aux_zc_weight)) return MOE_ERR_INVALID_ARG;   // NaN
+  if (c->opt_rows_fused < 0 || c->opt_rows_fused > 3 || c->opt_pair < 0 || c->opt_pair > 3 || c->opt_fp8_wide < 0 ||
+      c->opt_fp8_wide > 3 || c->opt_fp8_fused_quant < 0 || c->opt_fp8_fused_quant > 2)
+    return MOE_ERR_INVALID_ARG;
   return MOE_OK;
 }
 
@@ -47,9 +49,7 @@ bool rows_fusable(const moe_config_t* c) {
 
 int rows_fused(const moe_config_t* c) {
   if (!rows_fusable(c)) return 0;
-  const char* e = getenv("MOE_B200_FUSED_ROWS");      // read per call: tests flip it inside one process
-  if (e && e[0] >= '0' && e[0] <= '2') return e[0] - '0';
-  return 1;
+  return c->opt_rows_fused ? c->opt_rows_fused - 1 : 1;
 }
 
 int device_sm_count() {
@@ -138,8 +138,8 @@ WsLayout ws_layout(const moe_config_t* c) {
   L.dzp = k.take(R * 4);
   L.dwr_part = k.take((R / 128 + 1) * H * 4);   // per-tile partial sums of dWr (fp32)
   L.dy = k.take(R * H * es);                                 // fused rows: the UNWEIGHTED gathered dY
-  // reserved whenever the config COULD fuse, whatever MOE_B200_FUSED_ROWS says right now: every offset below must be the
-  // same for the sizing query, moe_layer_bwd and a later moe_layer_wgrad even if the knob changes between them
+  // reserved whenever the config COULD fuse, whatever cfg->opt_rows_fused says: every offset below must be the same for
+  // the sizing query, moe_layer_bwd and a later moe_layer_wgrad even if the caller changes the selector between them
   if (rows_fusable(c)) L.dwpart = k.take(2 * ((F + 255) / 256) * R * 4);
   L.dgu = k.take(R * 2 * F * es);
   L.dXp = k.take(R * H * es);

@@ -442,12 +442,12 @@ int32_t router_bwd_dense(const moe_config_t* c, const float* z, const int32_t* i
     TcCall g;
     if (dWr) {
       memset(&g, 0, sizeof(g));
-      g.mode = TC_WGRAD; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.M = E; g.A2 = X; g.lda2 = c->H; g.N = c->H;
+      g.mode = TC_WGRAD; g.opt_pair = c->opt_pair; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.M = E; g.A2 = X; g.lda2 = c->H; g.N = c->H;
       g.out0 = dWr; g.ld0 = c->H;
       MOE_CHECK(tc_gemm(g, s));
     }
     memset(&g, 0, sizeof(g));
-    g.mode = TC_DGRAD; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.B0 = Wr; g.b_rows = E; g.b_cols = c->H;
+    g.mode = TC_DGRAD; g.opt_pair = c->opt_pair; g.E = 1; g.rows_cap = c->T; g.A = dzb; g.lda = Ep; g.B0 = Wr; g.b_rows = E; g.b_cols = c->H;
     g.N = c->H; g.out0 = dXr; g.ld0 = c->H;
     return tc_gemm(g, s);
   }
@@ -462,7 +462,7 @@ int32_t router_logits(const moe_config_t* c, const void* X, const void* Wr, floa
   if (c->dtype != 0 && c->H % 64 == 0 && c->E % 4 == 0) {   // bf16: tcgen05 GEMM with fp32 output (one group of T rows)
     TcCall t;
     memset(&t, 0, sizeof(t));
-    t.mode = TC_FWD_F32; t.E = 1; t.rows_cap = c->T; t.A = X; t.lda = c->H; t.B0 = Wr; t.b_rows = c->E; t.b_cols = c->H;
+    t.mode = TC_FWD_F32; t.opt_pair = c->opt_pair; t.E = 1; t.rows_cap = c->T; t.A = X; t.lda = c->H; t.B0 = Wr; t.b_rows = c->E; t.b_cols = c->H;
     t.N = c->E; t.Kd = c->H; t.out0 = z; t.ld0 = c->E;
     const int32_t st = tc_gemm(t, s);
     if (st != MOE_ERR_UNSUPPORTED) return st;

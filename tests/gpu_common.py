@@ -50,6 +50,41 @@ def tile_gate(name, G, R, tol):
     return worst / tol
 
 
+def tile_gate_torch(name, G, R, tol):
+    """tile_gate for big tensors, evaluated on the device in torch fp64 (G: device tensor, R: the oracle's NumPy fp64 array):
+    the same two bounds, ~100x faster than NumPy on a 15 M-element weight gradient.  Returns (worst block ratio in units
+    of tol, ||G - R||_F / ||R||_F)."""
+    import torch
+    G = G.to(torch.float64)
+    R = torch.as_tensor(np.ascontiguousarray(R), dtype=torch.float64).to(G.device)
+    assert tuple(G.shape) == tuple(R.shape) and R.dim() == 2, (name, tuple(G.shape), tuple(R.shape))
+    if R.numel() == 0:
+        return 0.0, 0.0
+    rms = float(R.pow(2).mean().sqrt())
+    D = G - R
+    row_rms = R.pow(2).mean(dim=1, keepdim=True).sqrt()
+    bad = D.abs() > 6 * tol * torch.clamp(row_rms, min=rms) + tol * R.abs()
+    nbad = int(bad.sum())
+    if nbad:
+        ix = torch.nonzero(bad)[:6].tolist()
+        detail = [((i, j), float(G[i, j]), float(R[i, j]), float(row_rms[i, 0])) for i, j in ix]
+        raise AssertionError(f"{name}: {nbad} elements outside 6*tol*max(rms, row rms) + tol*|R| "
+                             f"(tol {tol}, rms {rms:.3e}; (index, got, want, row rms): {detail})")
+    nr, nc = -(-R.shape[0] // TILE_ROWS), -(-R.shape[1] // TILE_COLS)
+    pad = (0, nc * TILE_COLS - R.shape[1], 0, nr * TILE_ROWS - R.shape[0])
+    D2 = torch.nn.functional.pad(D * D, pad); R2 = torch.nn.functional.pad(R * R, pad)
+    dn = D2.reshape(nr, TILE_ROWS, nc, TILE_COLS).sum(dim=(1, 3)).sqrt()
+    rn = R2.reshape(nr, TILE_ROWS, nc, TILE_COLS).sum(dim=(1, 3)).sqrt()
+    assert not bool((dn[rn == 0] != 0).any()), f"{name}: non-zero output where the reference block is exactly zero"
+    floor = 0.05 * rms * np.sqrt(TILE_ROWS * TILE_COLS)
+    ratio = dn / torch.clamp(rn, min=floor)
+    worst = float(ratio.max())
+    assert worst <= 4 * tol, f"{name}: block rel err {worst:.3e} > 4*tol ({tol})"
+    nR = float(R.norm())
+    fro = float(D.norm()) / nR if nR > 0 else (0.0 if float(D.norm()) == 0 else float("inf"))
+    return worst / tol, fro
+
+
 def gen_inputs(cfg):
     X, dY, Wr, bias = wl.gen_X(cfg), wl.gen_dY(cfg), wl.gen_Wr(cfg), wl.gen_bias(cfg)
     W = wl.gen_all_expert_weights(cfg)

@@ -98,19 +98,24 @@ def test_layer_calls_reject_unsupported_configs_before_any_launch(moe):
     assert st == moe.MOE_ERR_UNSUPPORTED
 
 
-def test_ws_layout_does_not_depend_on_the_fusion_knob(moe, monkeypatch):
-    """The workspace size and every offset inside it are fixed by the config alone: MOE_B200_FUSED_ROWS may change between
-    the sizing query, moe_layer_bwd and a delayed moe_layer_wgrad without moving `dgu` / `dXp` (layout.cu)."""
-    cfg = wl.QWEN3_SMALL.replace(row_align=128)
+def test_ws_layout_does_not_depend_on_the_fusion_selector(moe):
+    """The workspace size and every offset inside it are fixed by the shape of the problem alone: opt_rows_fused may
+    differ between the sizing query, moe_layer_bwd and a delayed moe_layer_wgrad without moving `dgu` / `dXp` (ADVICE r2,
+    layout.cu).  Also: the library reads no environment variable any more."""
+    base = wl.QWEN3_SMALL.replace(row_align=128)
     seen = set()
-    for level in (None, "0", "1", "2"):
-        if level is None:
-            monkeypatch.delenv("MOE_B200_FUSED_ROWS", raising=False)
-        else:
-            monkeypatch.setenv("MOE_B200_FUSED_ROWS", level)
+    for sel in (0, 1, 2, 3):
+        cfg = base.replace(opt_rows_fused=sel)
+        assert moe.moe_layer_rows_fused(cfg) == (1 if sel == 0 else sel - 1)
         seen.add((moe.moe_workspace_bytes(cfg), moe.moe_ws_field(cfg, "dy"), moe.moe_ws_field(cfg, "dgu"),
                   moe.moe_ws_field(cfg, "dXp")))
     assert len(seen) == 1
+    with pytest.raises(moe.MoEError):
+        moe.moe_workspace_bytes(base.replace(opt_pair=4))
+    # (the static CUDA runtime inside the .so imports getenv for its own use, so the sources are what is checked)
+    csrc = os.path.join(ROOT, "paper_2605_31463_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
 
 
 def test_host_step_rejects_configs_that_need_extras_before_any_copy(moe):

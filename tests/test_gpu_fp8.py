@@ -127,15 +127,15 @@ def test_fp8_layer_fwd_bwd_matches_fake_quant_oracle(cfg):
     print(cfg.name, {k: (f"{v:.2e}" if isinstance(v, float) else v) for k, v in errs.items()})
 
 
-@pytest.mark.parametrize("fused", ["0", "1"])
+@pytest.mark.parametrize("fused", [0, 1])
 @pytest.mark.parametrize("mode", [0, 1])
-def test_fused_epilogue_quantisers_are_bit_exact(env, mode, fused, monkeypatch):
+def test_fused_epilogue_quantisers_are_bit_exact(env, mode, fused):
     """PAPER.md:116 fused FP8 quantisation: the codes and 1x128 scales that the GEMM-1 epilogue emits for `a` (Q-a) and
     the dgrad-down epilogue for [dg|du] (Q-dgu) are the SAME BITS the oracle's quantiser gives on the bf16 tensors those
     kernels wrote (rows of real tokens and padding rows; the shared expert's single-group path included)."""
     torch, moe, buffers = env
-    monkeypatch.setenv("MOE_B200_FP8_FUSED_QUANT", fused)      # "1": quantise in the epilogues; "0": stand-alone passes
-    cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode)
+    # opt_fp8_fused_quant = 2: quantise in the epilogues; = 1: stand-alone passes
+    cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode, opt_fp8_fused_quant=fused + 1)
     inp = gc.gen_inputs(cfg)
     lb = gc.run_gpu_layer(cfg, inp)
     gc.compare_layer(cfg, inp, lb)                              # ... and the layer still matches the fake-quant oracle
@@ -150,16 +150,14 @@ def test_fused_epilogue_quantisers_are_bit_exact(env, mode, fused, monkeypatch):
     assert np.array_equal(buffers.to_numpy(lb.ws_view("dguq_s"))[:R], sc)
 
 
-@pytest.mark.parametrize("wide", ["0", "2"])
-def test_fp8_tile_width_levels(env, wide, monkeypatch):
-    """The FP8 GEMMs run 128 x 256 tiles for the plain-epilogue modes by default (MOE_B200_FP8_WIDE=1; the other tests).
-    =0 keeps every GEMM on 128 x 128 tiles, =2 puts the fused-SwiGLU modes on the wide kernel too: same oracle, same
+@pytest.mark.parametrize("wide", [0, 2])
+def test_fp8_tile_width_levels(env, wide):
+    """The FP8 GEMMs run 128 x 256 tiles for the plain-epilogue modes by default (moe_config_t::opt_fp8_wide level 1; the other tests).
+    Level 0 keeps every GEMM on 128 x 128 tiles, level 2 puts the fused-SwiGLU modes on the wide kernel too: same oracle, same
     tolerance, and the fused quantisers' codes and scales stay bit-exact."""
     torch, moe, buffers = env
-    monkeypatch.setenv("MOE_B200_FP8_WIDE", wide)
-    monkeypatch.setenv("MOE_B200_FP8_FUSED_QUANT", "1")
     for mode in (0, 1):
-        cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode)
+        cfg = wl.DSV3_FP8_SMALL.replace(row_align=128, fp8_scale_mode=mode, opt_fp8_wide=wide + 1, opt_fp8_fused_quant=2)
         inp = gc.gen_inputs(cfg)
         lb = gc.run_gpu_layer(cfg, inp)
         gc.compare_layer(cfg, inp, lb)

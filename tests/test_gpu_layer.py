@@ -195,16 +195,16 @@ FUSED_CASES = [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128
 
 @pytest.mark.parametrize("level", [0, 2])
 @pytest.mark.parametrize("cfg", FUSED_CASES, ids=lambda c: c.name)
-def test_other_fusion_levels_match_oracle(cfg, level, monkeypatch):
+def test_other_fusion_levels_match_oracle(cfg, level):
     """bf16 layers default to moe_layer_rows_fused = 1 (routing weight in the GEMM-1 / dgrad-down epilogues, dw from the
-    dgrad-down epilogue; covered by test_layer_fwd_bwd_matches_oracle).  MOE_B200_FUSED_ROWS=0 keeps w in the combine and
-    the combine-backward pass, =2 also gathers the rows of X / dY inside the GEMMs (TMA tile::gather4) with Xp / dy as
+    dgrad-down epilogue; covered by test_layer_fwd_bwd_matches_oracle).  cfg.opt_rows_fused = 1 (level 0) keeps w in the combine and
+    the combine-backward pass, = 3 (level 2) also gathers the rows of X / dY inside the GEMMs (TMA tile::gather4) with Xp / dy as
     by-product copies: same oracle, same tolerance, and all three agree on the routing bit for bit."""
     import torch
     inp = gc.gen_inputs(cfg)
     dflt = gc.run_gpu_layer(cfg, inp)
     assert dflt.rows_fused == 1
-    monkeypatch.setenv("MOE_B200_FUSED_ROWS", str(level))
+    cfg = cfg.replace(opt_rows_fused=level + 1)
     lb = gc.run_gpu_layer(cfg, inp)
     assert lb.rows_fused == level
     errs = gc.compare_layer(cfg, inp, lb)
@@ -221,16 +221,16 @@ def test_fused_rows_query():
     assert moe.moe_layer_rows_fused(wl.DSV3_FP8_SMALL.replace(row_align=128)) == 0
 
 
-@pytest.mark.parametrize("pair", ["0", "2"])
+@pytest.mark.parametrize("pair", [0, 2])
 @pytest.mark.parametrize("cfg", [wl.QWEN3_SMALL.replace(name="qwen3_small_align128", row_align=128),
                                  wl.QWEN3_SMALL.replace(name="qwen3_small_align256", row_align=256),
                                  wl.GPTOSS_SMALL.replace(name="gptoss_small_align128", row_align=128)], ids=lambda c: c.name)
-def test_cta_pair_kernel_levels_match_oracle(cfg, pair, monkeypatch):
-    """MOE_B200_PAIR: 1 (default, the other tests) runs the weight gradients and single-group GEMMs on the cta_group::2 pair
+def test_cta_pair_kernel_levels_match_oracle(cfg, pair):
+    """moe_config_t::opt_pair (level + 1): level 1 (default, the other tests) runs the weight gradients and single-group GEMMs on the cta_group::2 pair
     kernel; 0 keeps every GEMM on the 1-CTA kernel; 2 also runs the ragged expert GEMMs as M-tile pairs (device-built
     pair / unpaired tile lists) followed by the 1-CTA kernel over the unpaired last tiles.  With row_align = 256 every
     tile is paired.  Same oracle, same tolerance."""
-    monkeypatch.setenv("MOE_B200_PAIR", pair)
+    cfg = cfg.replace(opt_pair=pair + 1)
     inp = gc.gen_inputs(cfg)
     lb = gc.run_gpu_layer(cfg, inp)
     errs = gc.compare_layer(cfg, inp, lb)

@@ -52,6 +52,11 @@ class MoEConfig:
     n_const: int = 0
     aux_coef: float = 0.0          # auxiliary load-balancing loss coefficient; 0 = off
     aux_zc_weight: float = 1.0     # weight of the zero-computation experts in the balance term
+    # kernel-variant selectors of moe_config_t (0 = the library default; v > 0 forces level v - 1; include/moe_b200.h)
+    opt_rows_fused: int = 0
+    opt_pair: int = 0
+    opt_fp8_wide: int = 0
+    opt_fp8_fused_quant: int = 0
     # input recipe only (not part of moe_config_t)
     w_std: float = 0.02            # expert weight std; <0 means 1/sqrt(fan_in) (configs[0])
     bias_kind: str = "none"        # "none" | "normal" (b~N(0,0.05)) | "zipf" (configs[4] skew offset)
