@@ -33,7 +33,7 @@ NOMINAL_FP8_OVER_BF16 = 2.0   # B200_PROFILING.md: 4.5 vs 2.25 PFLOP/s dense; th
 
 def load_traffic(workload):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's kernel, read from profiles/traffic.json
-    (written by `python -m paper_2605_31463_b200.ncu_summary` from an `ncu --set full` capture; it names the capture).
+    (written by `python ncu_summary.py` from an `ncu --set full` capture; it names the capture).
     Returns ({stage: bytes}, source string) or ({}, None) when no capture of this workload is tracked."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     try:

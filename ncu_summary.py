@@ -1,11 +1,11 @@
 """Turn Nsight Compute CSV exports of `bench.py` runs into the tracked summaries under profiles/.
 
-  python -m paper_2605_31463_b200.ncu_summary step RAW.csv --workload NAME --tag r2b --command "ncu ..."
+  python ncu_summary.py step RAW.csv --workload NAME --tag r2b --command "ncu ..."
       RAW.csv = `ncu -i REPORT.ncu-rep --page raw --csv` of an `ncu --set full` capture of one fwd+bwd step.
       Writes profiles/<tag>_step_<workload>.md (one line per launch: time, DRAM bytes, throughputs, tensor-pipe activity)
       and records dram__bytes_read.sum + dram__bytes_write.sum per launch of every GEMM stage in profiles/traffic.json,
       which bench.py reports as roofline.traffic.
-  python -m paper_2605_31463_b200.ncu_summary launches LAUNCHES.csv --tag r2b --command "ncu ..."
+  python ncu_summary.py launches LAUNCHES.csv --tag r2b --command "ncu ..."
       LAUNCHES.csv = the `--metrics gpu__time_duration.sum --csv --log-file` launch list.  Writes profiles/<tag>_launches.md.
 
 Reads text files only; runs nothing on a GPU."""
@@ -18,7 +18,7 @@ import json
 import os
 import re
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 PROFILES = os.path.join(ROOT, "profiles")
 TIME = {"ns": 1e-3, "nsecond": 1e-3, "us": 1.0, "usecond": 1.0, "ms": 1e3, "msecond": 1e3, "s": 1e6, "second": 1e6}
 BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
@@ -60,7 +60,7 @@ def cmd_step(a):
     rows = read_raw(a.csv)
     out = [f"# {a.tag}: `ncu --set full` capture of one whole fwd+bwd step, {a.workload}", "",
            "Command (on the B200 box, after the same bench command exited 0 without ncu); the CSV was exported on the box with",
-           "`ncu -i REPORT.ncu-rep --page raw --csv` and summarised here by `python -m paper_2605_31463_b200.ncu_summary step`:", "",
+           "`ncu -i REPORT.ncu-rep --page raw --csv` and summarised here by `python ncu_summary.py step`:", "",
            "```", a.command, "```", "",
            "| # | kernel | time us | dram read MB | dram write MB | dram thr % | L2 thr % | tensor pipe active % | regs | grid |",
            "|---|---|---|---|---|---|---|---|---|---|"]

@@ -92,7 +92,7 @@ def test_ncu_summary_parses_raw_and_launch_csv(tmp_path):
     """The script that writes profiles/*.md and profiles/traffic.json (bench.py's roofline.traffic) from ncu CSV exports:
     unit scaling, kernel naming, and the per-stage traffic (wgrad = mean of its three heaviest launches)."""
     import json
-    from paper_2605_31463_b200 import ncu_summary
+    import ncu_summary
     hdr = ["ID", "Kernel Name", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
            "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "lts__throughput.avg.pct_of_peak_sustained_elapsed",
            "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active", "launch__registers_per_thread", "launch__grid_size"]
